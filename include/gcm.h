@@ -1,0 +1,184 @@
+/*
+ * gcm.h -- C ABI of the B200-native AES-GCM engine (libb200gcm.so).
+ *
+ * The boundary follows the NIST SP 800-38D problem statement (the paper adopts it by reference,
+ * PAPER.md L111, L137, L255) and SURVEY.md section 8(b).  The hot path behind it is the one the
+ * paper's contribution targets: AES-CTR keystream XORed into the payload, fused with a GHASH over
+ * A || C || len computed as a parallel reduction with precomputed powers of H instead of the serial
+ * recurrence Y_i = (Y_{i-1} xor X_i) . H (Eq. 1; L272-L286, sections 5.2.1-5.2.2).
+ *
+ * Conventions
+ *   - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory on the
+ *     context's device (e.g. the data_ptr() of a torch uint8 tensor).  The library never allocates
+ *     or frees caller data.  A gcm_ctx owns its own device tables and scratch.
+ *   - Return codes follow the paper's Table 1 convention: 0 = success,
+ *     negative = argument / system error, positive = the operation ran but access was refused.
+ *   - IV is exactly 96 bits, tag exactly 128 bits (reading S5).
+ *   - len <= 2^36 - 32 bytes (SP 800-38D), aad_len < 2^61 bytes.  len = 0 and / or aad_len = 0 are
+ *     valid and the matching pointers may then be NULL (reading S6).
+ *   - In place (out == in) is allowed; any other overlap of in and out is GCM_ERR_ARG.
+ *   - Any byte alignment is accepted; the fast path needs `in` and `out` 16-byte aligned.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).
+ *   - A gcm_ctx may be used by one call at a time (it owns the cross-CTA scratch of that call).
+ *   - On GCM_ERR_AUTH the whole output [0, len) has been overwritten with zeros (the paper's payload
+ *     suppression) and the call completes normally (L245).  The fused kernel writes
+ *     plaintext before the tag is known (reading S9); the synchronous call does not return before
+ *     the compare and, on failure, the wipe have completed.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *     GCM_ERR_CUDA.
+ */
+#ifndef B200_GCM_H
+#define B200_GCM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GCM_API __attribute__((visibility("default")))
+#else
+#define GCM_API
+#endif
+
+typedef struct gcm_ctx gcm_ctx; /* opaque */
+
+enum {
+    GCM_OK        = 0,
+    GCM_ERR_AUTH  = 1,   /* tag mismatch: plaintext output has been zero-filled                 */
+    GCM_ERR_ARG   = -1,  /* NULL pointer, key_bits not 128/256, partial overlap, bad geometry    */
+    GCM_ERR_LEN   = -2,  /* len > 2^36 - 32 bytes, or aad_len >= 2^61 bytes                      */
+    GCM_ERR_CUDA  = -3,  /* CUDA runtime failure; see gcm_last_cuda_error()                      */
+    GCM_ERR_NOMEM = -4
+};
+
+/* Library / build identification: "b200gcm <version> sm_100a". Never NULL. */
+GCM_API const char *gcm_version(void);
+
+/* Selects the CUDA device (ordinal) used by subsequent gcm_init / batch calls of this thread's
+ * process.  Default 0.  Returns GCM_OK or GCM_ERR_CUDA. */
+GCM_API int gcm_set_device(int ordinal);
+
+/* Last cudaError_t seen by the library (0 = none), and its text (host, static storage). */
+GCM_API int gcm_last_cuda_error(void);
+GCM_API const char *gcm_last_cuda_error_string(void);
+
+/*
+ * gcm_init -- step a1 + a2 of SURVEY.md 8(a): key schedule (FIPS-197 5.2), H = E_K(0^128), the
+ * powers of H the reduction uses ("table of powers of the hash key",
+ * generated on the GPU) and the multiplier table of the fixed stride power.  Runs one setup
+ * kernel on the selected device.
+ *   out      (host, out)  receives the new context
+ *   key      (host)       16 or 32 bytes
+ *   key_bits              128 or 256 (reading S1); anything else -> GCM_ERR_ARG
+ */
+GCM_API int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits);
+
+/* Zeroises key material (device tables, host copy of the round keys) and frees the context.
+ * NULL is ignored. */
+GCM_API void gcm_destroy(gcm_ctx *ctx);
+
+/*
+ * Launch geometry of the fused kernel: `grid` CTAs (0 = one per SM) of `threads` threads (256 or
+ * 512; 0 = default 512).  The stride power H^(grid*threads) and its table are rebuilt.  Results
+ * never depend on the geometry (geometry-agnostic counters; reading S11).
+ * Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
+ */
+GCM_API int gcm_set_geometry(gcm_ctx *ctx, int grid, int threads);
+GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
+
+/* Copies the hash subkey H = E_K(0^128) (16 bytes) to host memory; for tests of step a2. */
+GCM_API int gcm_get_hash_subkey(const gcm_ctx *ctx, uint8_t h[16]);
+
+/*
+ * gcm_encrypt -- SURVEY.md 8(a) steps a3-a11, SP 800-38D Algorithm 4 (GCM-AE_K(IV, P, A)):
+ *   C = P xor E_K(IV || BE32(g + 2)) per 16-byte block g (counter from the block index only,
+ *   PAPER.md L259-L270); T = E_K(IV || 0^31 || 1) xor GHASH_H(A || 0* || C || 0* || len64(A) || len64(C)).
+ *   iv    (host)    12 bytes
+ *   d_aad (device)  aad_len bytes, may be NULL when aad_len = 0
+ *   d_pt  (device)  len bytes, may be NULL when len = 0
+ *   d_ct  (device)  len bytes, out
+ *   tag   (host)    16 bytes, out
+ * Synchronises `cuda_stream` before returning.
+ */
+GCM_API int gcm_encrypt(gcm_ctx *ctx, const uint8_t iv[12],
+                const void *d_aad, uint64_t aad_len,
+                const void *d_pt, uint64_t len,
+                void *d_ct, uint8_t tag[16], void *cuda_stream);
+
+/*
+ * gcm_decrypt_verify -- SP 800-38D Algorithm 5 (GCM-AD) with the paper's validation gate
+ * and payload suppression (L243): recomputes the tag from (IV, A, C), compares
+ * it with `tag` in constant time on the device, and returns GCM_OK with P in d_pt, or
+ * GCM_ERR_AUTH with d_pt[0..len) all zero.
+ *   tag   (host)    16 bytes, in
+ * Synchronises `cuda_stream` before returning.
+ */
+GCM_API int gcm_decrypt_verify(gcm_ctx *ctx, const uint8_t iv[12],
+                       const void *d_aad, uint64_t aad_len,
+                       const void *d_ct, uint64_t len,
+                       void *d_pt, const uint8_t tag[16], void *cuda_stream);
+
+/*
+ * Asynchronous forms for device-timed measurement (the paper's protocol places cudaEvent pairs
+ * strictly around the kernels): same computation, tag / status stay on the device,
+ * no synchronisation, no host transfer.
+ *   d_tag    (device) 16 bytes: out for encrypt, in (expected tag) for decrypt
+ *   d_status (device) one int32: GCM_OK or GCM_ERR_AUTH; on GCM_ERR_AUTH d_pt is zero-filled by a
+ *            wipe kernel enqueued on the same stream.
+ */
+GCM_API int gcm_encrypt_async(gcm_ctx *ctx, const uint8_t iv[12],
+                      const void *d_aad, uint64_t aad_len,
+                      const void *d_pt, uint64_t len,
+                      void *d_ct, void *d_tag, void *cuda_stream);
+
+GCM_API int gcm_decrypt_verify_async(gcm_ctx *ctx, const uint8_t iv[12],
+                             const void *d_aad, uint64_t aad_len,
+                             const void *d_ct, uint64_t len,
+                             void *d_pt, const void *d_tag, void *d_status, void *cuda_stream);
+
+/*
+ * GHASH only (GMAC-style measurement; the paper's Table 5 "GHashKernelOnly",
+ * PAPER.md L363, L379-L392): S = GHASH_H(A || 0* || C || 0* || len64(A) || len64(C)) over
+ * device-resident data, 16 bytes written to d_out (device).  No AES on the payload.
+ */
+GCM_API int gcm_ghash_async(gcm_ctx *ctx, const void *d_aad, uint64_t aad_len,
+                    const void *d_c, uint64_t len, void *d_out, void *cuda_stream);
+
+/*
+ * Batched many-message variant (FITS-sized HDUs and many short messages).
+ * One descriptor per message; keys may differ per message.
+ *   key      (host)   16 or 32 bytes       key_bits 128 or 256
+ *   iv                12 bytes
+ *   d_aad    (device) aad_len bytes        d_in / d_out (device) len bytes
+ *   tag               out (encrypt) / in (decrypt)
+ *   status            per message: GCM_OK / GCM_ERR_AUTH / negative error
+ * gcm_encrypt_batch returns GCM_OK or the first negative error.
+ * gcm_decrypt_verify_batch returns the number of messages that failed authentication (their
+ * outputs are zero-filled) or a negative error.  Both synchronise `cuda_stream`.
+ */
+typedef struct {
+    const uint8_t *key;
+    int            key_bits;
+    uint8_t        iv[12];
+    const void    *d_aad;
+    uint64_t       aad_len;
+    const void    *d_in;
+    uint64_t       len;
+    void          *d_out;
+    uint8_t        tag[16];
+    int            status;
+} gcm_msg;
+
+GCM_API int gcm_encrypt_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
+GCM_API int gcm_decrypt_verify_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
+
+/* Frees the batch path's cached per-key contexts and staging buffers (zeroising key material). */
+GCM_API void gcm_batch_release(void);
+
+#ifdef __cplusplus
+}
+#endif
+
+#endif /* B200_GCM_H */

@@ -1,0 +1,323 @@
+// gcm_api.cu -- the C ABI of libb200gcm.so (include/gcm.h): argument checks, launch parameters,
+// context ownership.  No arithmetic of the method runs on the host: key schedule, H, powers,
+// CTR, GHASH, tag and compare are all kernels (gcm_setup.cu, gcm_fused.cu, gcm_batch.cu).
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+#include <stdlib.h>
+#include <new>
+
+#include "../../include/gcm.h"
+#include "gcm_common.cuh"
+#include "gcm_setup.cuh"
+#include "gcm_fused.cuh"
+#include "gcm_api_internal.h"
+
+static int g_device = 0;
+static int g_last_cuda_error = 0;
+
+int gcm_cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    cudaGetLastError();   // clear the sticky-free error state
+    return e == cudaErrorMemoryAllocation ? GCM_ERR_NOMEM : GCM_ERR_CUDA;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
+    } while (0)
+
+extern "C" const char *gcm_version(void) { return "b200gcm 0.1 sm_100a"; }
+
+extern "C" int gcm_set_device(int ordinal)
+{
+    CU(cudaSetDevice(ordinal));
+    g_device = ordinal;
+    return GCM_OK;
+}
+
+extern "C" int gcm_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" const char *gcm_last_cuda_error_string(void)
+{
+    return cudaGetErrorString((cudaError_t)g_last_cuda_error);
+}
+
+static void secure_zero(void *p, size_t n)
+{
+    volatile uint8_t *v = (volatile uint8_t *)p;
+    while (n--) *v++ = 0;
+}
+
+static SetupParams setup_params(gcm_ctx *c, const uint8_t *key)
+{
+    SetupParams sp;
+    memset(&sp, 0, sizeof(sp));
+    if (key) memcpy(sp.key, key, c->key_bits / 8);
+    sp.key_bits = c->key_bits;
+    sp.threads = c->threads;
+    sp.grid = c->grid;
+    sp.te0 = c->d_te0;
+    sp.rk = c->d_rk;
+    sp.h = c->d_h;
+    sp.hpow = c->d_hpow;
+    sp.bpow = c->d_bpow;
+    sp.ktab = c->d_ktab;
+    return sp;
+}
+
+extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
+{
+    if (!out || !key || (key_bits != 128 && key_bits != 256)) return GCM_ERR_ARG;
+    *out = nullptr;
+    CU(cudaSetDevice(g_device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, g_device));
+    if ((size_t)prop.sharedMemPerBlockOptin < (size_t)FUSED_SMEM_BYTES) return GCM_ERR_CUDA;
+
+    gcm_ctx *c = new (std::nothrow) gcm_ctx;
+    if (!c) return GCM_ERR_NOMEM;
+    memset(c, 0, sizeof(*c));
+    c->device = g_device;
+    c->key_bits = key_bits;
+    c->nr = key_bits == 128 ? 10 : 14;
+    c->sm_count = prop.multiProcessorCount;
+    c->grid = c->sm_count;
+    c->threads = GCM_MAX_THREADS;
+
+    // one slab for all device-side state
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    size_t o_te0 = take(256 * 4), o_rk = take(64 * 4), o_h = take(16);
+    size_t o_hpow = take((GCM_MAX_THREADS + 1) * 16), o_bpow = take((GCM_MAX_GRID + 1) * 16);
+    size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
+    size_t o_cnt = take(4), o_tag = take(16), o_status = take(4);
+    c->slab_bytes = off;
+    cudaError_t e = cudaMalloc((void **)&c->d_slab, c->slab_bytes);
+    if (e != cudaSuccess) { delete c; return gcm_cuda_fail(e); }
+    c->d_te0 = (uint32_t *)(c->d_slab + o_te0);
+    c->d_rk = (uint32_t *)(c->d_slab + o_rk);
+    c->d_h = (uint4 *)(c->d_slab + o_h);
+    c->d_hpow = (uint4 *)(c->d_slab + o_hpow);
+    c->d_bpow = (uint4 *)(c->d_slab + o_bpow);
+    c->d_ktab = (uint4 *)(c->d_slab + o_ktab);
+    c->d_partials = (uint4 *)(c->d_slab + o_part);
+    c->d_counter = (unsigned *)(c->d_slab + o_cnt);
+    c->d_tag = (uint4 *)(c->d_slab + o_tag);
+    c->d_status = (int *)(c->d_slab + o_status);
+
+    int rc = GCM_OK;
+    do {
+        if ((e = cudaHostAlloc((void **)&c->h_pinned, 64, cudaHostAllocDefault)) != cudaSuccess) break;
+        if ((e = cudaMemset(c->d_slab, 0, c->slab_bytes)) != cudaSuccess) break;
+        SetupParams sp = setup_params(c, key);
+        launch_setup(sp, 0);
+        secure_zero(&sp, sizeof(sp));
+        if ((e = cudaGetLastError()) != cudaSuccess) break;
+        if ((e = cudaMemcpy(c->h_rk, c->d_rk, sizeof(c->h_rk), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+    } while (0);
+    if (e != cudaSuccess) {
+        rc = gcm_cuda_fail(e);
+        gcm_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return GCM_OK;
+}
+
+extern "C" void gcm_destroy(gcm_ctx *c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    if (c->d_slab) {
+        launch_wipe(c->d_slab, c->slab_bytes, nullptr, 0);
+        cudaDeviceSynchronize();
+        cudaFree(c->d_slab);
+    }
+    if (c->h_pinned) {
+        secure_zero(c->h_pinned, 64);
+        cudaFreeHost(c->h_pinned);
+    }
+    cudaGetLastError();
+    secure_zero(c, sizeof(*c));
+    delete c;
+}
+
+extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)
+{
+    if (!c) return GCM_ERR_ARG;
+    if (grid == 0) grid = c->sm_count;
+    if (threads == 0) threads = GCM_MAX_THREADS;
+    if (grid < 1 || grid > GCM_MAX_GRID || (threads != 256 && threads != 512)) return GCM_ERR_ARG;
+    CU(cudaSetDevice(c->device));
+    if (grid == c->grid && threads == c->threads) return GCM_OK;
+    c->grid = grid;
+    c->threads = threads;
+    SetupParams sp = setup_params(c, nullptr);
+    launch_regeometry(sp, 0);
+    CU(cudaGetLastError());
+    CU(cudaDeviceSynchronize());
+    return GCM_OK;
+}
+
+extern "C" int gcm_get_geometry(const gcm_ctx *c, int *grid, int *threads)
+{
+    if (!c) return GCM_ERR_ARG;
+    if (grid) *grid = c->grid;
+    if (threads) *threads = c->threads;
+    return GCM_OK;
+}
+
+extern "C" int gcm_get_hash_subkey(const gcm_ctx *c, uint8_t h[16])
+{
+    if (!c || !h) return GCM_ERR_ARG;
+    CU(cudaSetDevice(c->device));
+    CU(cudaMemcpy(h, c->d_h, 16, cudaMemcpyDeviceToHost));
+    return GCM_OK;
+}
+
+// Argument checks and launch parameters common to encrypt / decrypt / ghash.
+static int build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
+                        const void *d_in, uint64_t len, void *d_out, GcmParams *p, int *blocks)
+{
+    if (!c) return GCM_ERR_ARG;
+    if (mode != MODE_GHASH && !iv) return GCM_ERR_ARG;
+    if (len > ((1ull << 36) - 32) || aad_len >= (1ull << 61)) return GCM_ERR_LEN;
+    if ((aad_len && !d_aad) || (len && !d_in)) return GCM_ERR_ARG;
+    if (mode != MODE_GHASH && len && !d_out) return GCM_ERR_ARG;
+    const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+    if (mode != MODE_GHASH && len && a != b && a < b + len && b < a + len) return GCM_ERR_ARG;  // partial overlap
+
+    memset(p, 0, sizeof(*p));
+    memcpy(p->rk, c->h_rk, sizeof(p->rk));
+    if (iv) {
+        memcpy(p->iv, iv, 12);
+        for (int i = 0; i < 3; i++) p->iv_rk0[i] = p->iv[i] ^ p->rk[i];
+    }
+    p->in = (const uint8_t *)d_in;
+    p->out = (uint8_t *)d_out;
+    p->aad = (const uint8_t *)d_aad;
+    p->len = len;
+    p->aad_len = aad_len;
+    p->n_full = len / 16;
+    const uint64_t n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
+    const uint64_t T = (uint64_t)c->threads;
+    const uint64_t total = n_blocks + n_aad;
+    const uint64_t rows = (total + T - 1) / T;
+    if (n_aad > 0xFFFFFFFFull || rows > 0xFFFFFFFFull) return GCM_ERR_LEN;
+    p->rows = (uint32_t)rows;
+    p->pad = (uint32_t)(rows * T - total);
+    p->n_aad_blocks = (uint32_t)n_aad;
+    p->base = (uint64_t)p->pad + n_aad;
+    p->grid_stride = (uint32_t)c->grid;
+    p->aligned = (((a | (mode == MODE_GHASH ? 0 : b)) & 15) == 0) ? 1u : 0u;
+    if (p->aligned) {
+        p->fast_lo = (uint32_t)((p->base + T - 1) / T);
+        p->fast_hi = (uint32_t)((p->n_full + p->base) / T);
+        if (p->fast_hi < p->fast_lo) p->fast_hi = p->fast_lo;
+    }
+    p->tab.te0 = c->d_te0;
+    p->tab.ktab = c->d_ktab;
+    p->tab.hpow = c->d_hpow;
+    p->tab.bpow = c->d_bpow;
+    p->tab.h = c->d_h;
+    p->partials = c->d_partials;
+    p->counter = c->d_counter;
+    p->tag_out = c->d_tag;
+    p->status = c->d_status;
+    uint64_t want = rows < 1 ? 1 : rows;
+    *blocks = (int)(want < (uint64_t)c->grid ? want : (uint64_t)c->grid);
+    return GCM_OK;
+}
+
+extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                                 const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
+{
+    GcmParams p;
+    int blocks = 0;
+    if (!d_tag) return GCM_ERR_ARG;
+    int rc = build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    p.tag_out = (uint4 *)d_tag;
+    CU(cudaSetDevice(c->device));
+    cudaError_t e = launch_fused(c->nr, MODE_ENCRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    return GCM_OK;
+}
+
+extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                                        const void *d_ct, uint64_t len, void *d_pt, const void *d_tag,
+                                        void *d_status, void *stream)
+{
+    GcmParams p;
+    int blocks = 0;
+    if (!d_tag || !d_status) return GCM_ERR_ARG;
+    int rc = build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    p.tag_in = (const uint4 *)d_tag;
+    p.status = (int *)d_status;
+    CU(cudaSetDevice(c->device));
+    cudaError_t e = launch_fused(c->nr, MODE_DECRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    // validation gate + payload suppression (L243), decided on the device
+    launch_wipe((uint8_t *)d_pt, len, (const int *)d_status, (cudaStream_t)stream);
+    CU(cudaGetLastError());
+    return GCM_OK;
+}
+
+extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, const void *d_c, uint64_t len,
+                               void *d_out, void *stream)
+{
+    GcmParams p;
+    int blocks = 0;
+    if (!d_out) return GCM_ERR_ARG;
+    int rc = build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    p.tag_out = (uint4 *)d_out;
+    CU(cudaSetDevice(c->device));
+    cudaError_t e = launch_fused(c->nr, MODE_GHASH, c->threads, blocks, p, (cudaStream_t)stream);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    return GCM_OK;
+}
+
+extern "C" int gcm_encrypt(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                           const void *d_pt, uint64_t len, void *d_ct, uint8_t tag[16], void *stream)
+{
+    if (!c || !tag) return GCM_ERR_ARG;
+    int rc = gcm_encrypt_async(c, iv, d_aad, aad_len, d_pt, len, d_ct, c->d_tag, stream);
+    if (rc != GCM_OK) return rc;
+    CU(cudaMemcpyAsync(c->h_pinned, c->d_tag, 16, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    memcpy(tag, c->h_pinned, 16);
+    return GCM_OK;
+}
+
+extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                                  const void *d_ct, uint64_t len, void *d_pt, const uint8_t tag[16], void *stream)
+{
+    if (!c || !tag) return GCM_ERR_ARG;
+    GcmParams p;
+    int blocks = 0;
+    int rc = build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
+    CU(cudaSetDevice(c->device));
+    cudaError_t e = launch_fused(c->nr, MODE_DECRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    CU(cudaMemcpyAsync(c->h_pinned + 16, c->d_status, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    int status;
+    memcpy(&status, c->h_pinned + 16, 4);
+    if (status != 0) {
+        launch_wipe((uint8_t *)d_pt, len, nullptr, (cudaStream_t)stream);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize((cudaStream_t)stream));
+        return GCM_ERR_AUTH;
+    }
+    return GCM_OK;
+}

@@ -1,0 +1,31 @@
+// gcm_api_internal.h -- the context behind the opaque gcm_ctx of include/gcm.h (host side only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+struct gcm_ctx {
+    int device;
+    int key_bits;
+    int nr;            // 10 / 14
+    int sm_count;
+    int grid;          // G: CTAs of the fused kernel (default: one per SM)
+    int threads;       // T: threads per CTA (512 default, 256 alternative)
+    // device state, one slab
+    uint8_t  *d_slab;
+    size_t    slab_bytes;
+    uint32_t *d_te0;
+    uint32_t *d_rk;
+    uint4    *d_h;
+    uint4    *d_hpow;
+    uint4    *d_bpow;
+    uint4    *d_ktab;
+    uint4    *d_partials;
+    unsigned *d_counter;
+    uint4    *d_tag;
+    int      *d_status;
+    // host state
+    uint32_t  h_rk[60];   // round keys (little-endian column words) for the kernel parameter block
+    uint8_t  *h_pinned;   // 64 bytes of pinned memory: tag [0,16), status [16,20)
+};
+
+int gcm_cuda_fail(cudaError_t e);

@@ -1,0 +1,67 @@
+// gcm_common.cuh -- constants, table layouts and launch-parameter structs shared by the kernels
+// and the host side of libb200gcm.so.  Shares nothing with oracle/.
+#pragma once
+#include <stdint.h>
+
+// ---- shared-memory layout of the fused kernel (bytes) -------------------------------------------
+// AES round tables, laid out so that every lane of a warp owns one 4-byte bank (conflict-free AND
+// constant-time for secret indices).  Row x (x = S-box input, 0..255) is 256 bytes:
+//     A0: [T0[x] for lanes 0..31][T1[x] for lanes 0..31]      A1: [T2[x] ..][T3[x] ..]
+// so the byte address of T_k[x] for a lane is  x*256 + lane*4 (+128 for the odd table): one PRMT
+// builds it from the state byte and the lane offset, no shift / multiply needed.
+#define AES_A0_OFF      0
+#define AES_A1_OFF      65536
+#define AES_ODD_OFF     128
+#define AES_TAB_BYTES   131072
+// GHASH multiplier table for the fixed stride power K = H^(grid*threads): 8-bit Shoup tables, one
+// per byte position P = 0..15.  Entry (P, v) = (block with byte P = v, zero elsewhere) . K, 16 bytes
+// in memory byte order, stored at  v*256 + (P>>3)*128 + (P&7)*16.  Within a quarter-warp lane q
+// visits positions in the rotated order (q + r) & 7, so the eight 16-byte accesses of one LDS.128
+// phase fall into eight distinct bank groups: conflict-free without replication.
+#define KTAB_OFF        131072
+#define KTAB_BYTES      65536
+#define RED_OFF         (KTAB_OFF + KTAB_BYTES)     /* cross-warp reduction scratch: 32 x 16 B */
+#define RED_BYTES       512
+#define FUSED_SMEM_BYTES (RED_OFF + RED_BYTES)
+
+#define GCM_MAX_THREADS 512
+#define GCM_MAX_GRID    4096
+
+enum { MODE_ENCRYPT = 0, MODE_DECRYPT = 1, MODE_GHASH = 2 };
+
+// Device-resident per-key tables (owned by gcm_ctx).
+struct GcmTables {
+    const uint32_t *te0;     // 256 words: T0[x] = {02.S, S, S, 03.S} (little-endian word, row 0 low)
+    const uint4    *ktab;    // KTAB_BYTES, layout above
+    const uint4    *hpow;    // hpow[i] = H^i, i = 0..threads ("mem" format)
+    const uint4    *bpow;    // bpow[j] = (H^threads)^j, j = 0..grid
+    const uint4    *h;       // H
+};
+
+// Kernel parameters, passed by value (constant bank): the round keys are then free operands of
+// the XOR instructions.
+struct GcmParams {
+    uint32_t rk[60];         // round keys, little-endian column words: rk[4r + c]
+    uint32_t iv_rk0[3];      // IV words ^ rk[0..2]: columns 0..2 of every counter block after AddRoundKey(0)
+    uint32_t iv[3];          // IV words (little-endian load of bytes 0..11)
+    const uint8_t *in;
+    uint8_t       *out;
+    const uint8_t *aad;
+    uint64_t len;            // payload bytes
+    uint64_t aad_len;
+    uint64_t n_full;         // floor(len / 16)
+    uint64_t base;           // pad + n_aad_blocks: virtual index of payload block 0
+    uint32_t pad;            // leading virtual zero blocks (rows*threads - n_aad_blocks - n_blocks)
+    uint32_t n_aad_blocks;
+    uint32_t rows;           // R: virtual blocks / threads
+    uint32_t grid_stride;    // G: rows are dealt round-robin to G CTAs (the table's stride power is H^(G*threads))
+    uint32_t fast_lo, fast_hi; // rows [fast_lo, fast_hi) hold only whole, aligned payload blocks
+    uint32_t aligned;        // in and out are 16-byte aligned
+    GcmTables tab;
+    uint4    *partials;      // one per CTA
+    unsigned *counter;       // last-CTA-done ticket
+    uint4    *tag_out;       // device, 16 bytes (encrypt: tag; ghash mode: S)
+    const uint4 *tag_in;     // device, 16 bytes or NULL -> tag_expect below
+    uint32_t tag_expect[4];
+    int      *status;        // device
+};

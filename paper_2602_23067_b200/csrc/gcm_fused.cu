@@ -1,0 +1,308 @@
+// gcm_fused.cu -- the hot path: SURVEY.md 8(a) steps a3-a11 in ONE kernel.
+//
+//   AES-CTR keystream (a4, a5) -> XOR into the payload (a6) -> GHASH of the ciphertext while it is
+//   still in registers (a7) -> per-thread / CTA / cross-CTA combination with precomputed powers of
+//   H (a8, a9) -> AAD + length block, E_K(J0), tag, constant-time compare
+//   (a10, a11).
+//
+// What differs from the paper's kernels (prior art for Ampere/Ada/Hopper):
+//   * one fused pass instead of an AES-CTR kernel followed by a GHASH kernel (the ciphertext never
+//     crosses HBM twice);
+//   * the "tree" is flattened: virtual block v = row*T + t (T threads per CTA, rows dealt round-robin
+//     to the G CTAs) so every thread runs the SAME recurrence  Y <- Y.K xor X  with the one fixed
+//     multiplier K = H^(G*T), then is corrected once by H^(T-t), the CTA by (H^T)^e, and the CTA
+//     partials are XORed by the last CTA to finish.  The sum is the paper's sum of X_i . H^(N-i+1);
+//     only the association differs, and the field is exact, so the bits are identical;
+//   * the multiply by the fixed K is an 8-bit Shoup table in shared memory (conflict-free by lane
+//     rotation), AES rounds are T-tables replicated per lane (conflict-free, constant-time).  On
+//     sm_100a the binding unit is the shared-memory pipe: 16*NR + 64 wavefront-lanes per block.
+//
+// Counter block of payload block g is IV || BE32(g + 2): a function of g only.
+#include "gcm_common.cuh"
+#include "gf128.cuh"
+#include "gcm_fused.cuh"
+
+__device__ __forceinline__ uint32_t lds32(const uint8_t *sm, uint32_t off)
+{
+    return *reinterpret_cast<const uint32_t *>(sm + off);
+}
+__device__ __forceinline__ uint4 lds128(const uint8_t *sm, uint32_t off)
+{
+    return *reinterpret_cast<const uint4 *>(sm + off);
+}
+__device__ __forceinline__ uint32_t rotl32(uint32_t x, int n) { return __funnelshift_l(x, x, n); }
+
+// byte address of row (state byte `row` of w) in this lane's bank column: one PRMT
+#define TIDX(w, row) __byte_perm((w), lane4, 0x5504u | ((row) << 4))
+
+// Rounds 1..NR on a state that already had AddRoundKey(0) applied.  Little-endian column words.
+template <int NR>
+__device__ __forceinline__ uint4 aes_rounds(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
+                                            uint32_t s0, uint32_t s1, uint32_t s2, uint32_t s3)
+{
+    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
+#pragma unroll
+    for (int r = 1; r < NR; r++) {
+        uint32_t t0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[4 * r + 0];
+        uint32_t t1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[4 * r + 1];
+        uint32_t t2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[4 * r + 2];
+        uint32_t t3 = lds32(sm, TIDX(s3, 0) + T0) ^ lds32(sm, TIDX(s0, 1) + T1) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[4 * r + 3];
+        s0 = t0; s1 = t1; s2 = t2; s3 = t3;
+    }
+    // Final round (no MixColumns): S(x) sits in byte 0 of T2[x], bytes 1 and 2 of T0[x], byte 3 of T1[x].
+    uint4 o;
+#define FINAL(a, b, c, d, k)                                                                       \
+    (__byte_perm(__byte_perm(lds32(sm, TIDX(a, 0) + T2), lds32(sm, TIDX(b, 1) + T0), 0x0050),      \
+                 __byte_perm(lds32(sm, TIDX(c, 2) + T0), lds32(sm, TIDX(d, 3) + T1), 0x7200), 0x7610) ^ p.rk[4 * NR + (k)])
+    o.x = FINAL(s0, s1, s2, s3, 0);
+    o.y = FINAL(s1, s2, s3, s0, 1);
+    o.z = FINAL(s2, s3, s0, s1, 2);
+    o.w = FINAL(s3, s0, s1, s2, 3);
+#undef FINAL
+    return o;
+}
+
+// y . K for the fixed stride power K: sixteen 16-byte table entries XORed (a7).  sel[r] =
+// ((lane + r) & 7) << 4 is both the PRMT selector that moves byte (lane + r) & 7 of the 8-byte half
+// into address byte 1 and the 16-byte column offset of that position inside the 128-byte half-row.
+__device__ __forceinline__ uint4 ghash_mul_k(const uint8_t *sm, const uint32_t (&sel)[8], uint4 y)
+{
+    uint4 acc = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int r = 0; r < 8; r++) {
+        uint32_t off = (__byte_perm(y.x, y.y, sel[r]) & 0xFF00u) | sel[r];
+        acc = xor4(acc, lds128(sm, KTAB_OFF + off));
+    }
+#pragma unroll
+    for (int r = 0; r < 8; r++) {
+        uint32_t off = (__byte_perm(y.z, y.w, sel[r]) & 0xFF00u) | sel[r];
+        acc = xor4(acc, lds128(sm, KTAB_OFF + 128 + off));
+    }
+    return acc;
+}
+
+__device__ __forceinline__ uint4 ld16_stream(const uint8_t *p)
+{
+    return __ldcs(reinterpret_cast<const uint4 *>(p));
+}
+__device__ __forceinline__ void st16_stream(uint8_t *p, uint4 v)
+{
+    __stcs(reinterpret_cast<uint4 *>(p), v);
+}
+
+// n (0..16) bytes -> block, zero-padded (a ragged tail, an unaligned buffer, an AAD block)
+static __device__ __noinline__ uint4 load_bytes(const uint8_t *p, uint32_t n)
+{
+    uint32_t w[4] = {0, 0, 0, 0};
+    for (uint32_t i = 0; i < n; i++) w[i >> 2] |= (uint32_t)p[i] << (8 * (i & 3));
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
+static __device__ __noinline__ void store_bytes(uint8_t *p, uint4 v, uint32_t n)
+{
+    uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    for (uint32_t i = 0; i < n; i++) p[i] = (uint8_t)(w[i >> 2] >> (8 * (i & 3)));
+}
+// keep the first n bytes, zero the rest (GHASH sees the ciphertext zero-padded, never keystream)
+__device__ __forceinline__ uint4 keep_bytes(uint4 v, uint32_t n)
+{
+    uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        int nb = (int)n - 4 * k;
+        uint32_t m = nb >= 4 ? 0xFFFFFFFFu : (nb <= 0 ? 0u : ((1u << (8 * nb)) - 1u));
+        w[k] &= m;
+    }
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
+
+// XOR of v over the CTA; result valid in thread 0.  red: 32 x uint4 of shared memory.
+__device__ __forceinline__ uint4 cta_xor_reduce(uint4 v, uint4 *red)
+{
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        v.x ^= __shfl_xor_sync(0xFFFFFFFFu, v.x, o); v.y ^= __shfl_xor_sync(0xFFFFFFFFu, v.y, o);
+        v.z ^= __shfl_xor_sync(0xFFFFFFFFu, v.z, o); v.w ^= __shfl_xor_sync(0xFFFFFFFFu, v.w, o);
+    }
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = lane < nwarps ? red[lane] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            v.x ^= __shfl_xor_sync(0xFFFFFFFFu, v.x, o); v.y ^= __shfl_xor_sync(0xFFFFFFFFu, v.y, o);
+            v.z ^= __shfl_xor_sync(0xFFFFFFFFu, v.z, o); v.w ^= __shfl_xor_sync(0xFFFFFFFFu, v.w, o);
+        }
+    }
+    __syncthreads();
+    return v;
+}
+
+template <int TPB>
+__device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const uint32_t *te0)
+{
+    uint32_t *a0 = reinterpret_cast<uint32_t *>(sm + AES_A0_OFF);
+    uint32_t *a1 = reinterpret_cast<uint32_t *>(sm + AES_A1_OFF);
+    for (uint32_t j = threadIdx.x; j < 16384; j += TPB) {
+        uint32_t te = __ldg(te0 + (j >> 6));
+        bool odd = (j >> 5) & 1;
+        a0[j] = odd ? rotl32(te, 8) : te;            // T0 | T1
+        a1[j] = odd ? rotl32(te, 24) : rotl32(te, 16); // T2 | T3
+    }
+}
+
+template <int NR, int MODE, int TPB>
+__global__ void __launch_bounds__(TPB, 1)
+gcm_fused_kernel(const __grid_constant__ GcmParams p)
+{
+    extern __shared__ __align__(1024) uint8_t sm[];
+    __shared__ bool s_last;
+    const uint32_t t = threadIdx.x, lane = t & 31, lane4 = lane * 4;
+    const uint32_t G = p.grid_stride, c = blockIdx.x;
+    const bool active = c < p.rows;
+    uint4 *red = reinterpret_cast<uint4 *>(sm + RED_OFF);
+
+    if (active) {
+        if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
+        uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
+        for (uint32_t j = t; j < KTAB_BYTES / 16; j += TPB) kt[j] = __ldg(p.tab.ktab + j);
+    }
+    __syncthreads();
+
+    uint32_t sel[8];
+#pragma unroll
+    for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
+
+    uint4 Y = make_uint4(0, 0, 0, 0);
+    uint4 pre = make_uint4(0, 0, 0, 0);
+    bool have_pre = false;
+    const uint64_t row_bytes = (uint64_t)G * TPB * 16;
+
+    for (uint32_t row = c; row < p.rows; row += G) {
+        const uint64_t v = (uint64_t)row * TPB + t;     // virtual block index
+        const bool fast = row >= p.fast_lo && row < p.fast_hi;
+        uint4 x = make_uint4(0, 0, 0, 0);
+        uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD)
+        uint64_t g = 0;                                 // payload block index
+        if (fast) {
+            g = v - p.base;
+            x = have_pre ? pre : ld16_stream(p.in + 16 * g);
+            cbytes = 16;
+            have_pre = row + G < p.fast_hi;
+            if (have_pre) pre = ld16_stream(p.in + 16 * g + row_bytes);
+        } else {
+            have_pre = false;
+            if (v >= p.pad) {
+                const uint64_t u = v - p.pad;
+                if (u < p.n_aad_blocks) {
+                    const uint64_t rem = p.aad_len - 16 * u;
+                    x = load_bytes(p.aad + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
+                } else {
+                    g = u - p.n_aad_blocks;
+                    const uint64_t rem = p.len - 16 * g;
+                    cbytes = rem < 16 ? (uint32_t)rem : 16u;
+                    x = (cbytes == 16 && p.aligned) ? ld16_stream(p.in + 16 * g) : load_bytes(p.in + 16 * g, cbytes);
+                }
+            }
+        }
+        // a7: multiply the running value by K; independent of this row's AES, so they interleave
+        const uint4 ym = ghash_mul_k(sm, sel, Y);
+        uint4 X = x;
+        if (MODE != MODE_GHASH) {
+            // a4 + a5: counter from the block index, then the rounds
+            const uint32_t s3 = bswap32((uint32_t)g + 2u) ^ p.rk[3];
+            const uint4 ks = aes_rounds<NR>(p, sm, lane4, p.iv_rk0[0], p.iv_rk0[1], p.iv_rk0[2], s3);
+            const uint4 y = xor4(x, ks);                                   // a6
+            if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
+            else if (cbytes) store_bytes(p.out + 16 * g, y, cbytes);
+            if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
+        }
+        Y = xor4(ym, X);
+    }
+
+    // a8: per-thread correction by H^(T - t), XOR over the CTA, CTA correction by (H^T)^e
+    uint4 part = make_uint4(0, 0, 0, 0);
+    if (active) {
+        const uint4 yc = gf_mul_mem(Y, __ldg(p.tab.hpow + (TPB - t)));
+        part = cta_xor_reduce(yc, red);
+        if (t == 0) {
+            const uint32_t last = c + G * ((p.rows - 1 - c) / G);
+            const uint32_t e = p.rows - 1 - last;
+            if (e) part = gf_mul_mem(part, __ldg(p.tab.bpow + e));
+        }
+    }
+    // a9: last-CTA-done combination of the partials
+    if (t == 0) {
+        p.partials[c] = part;
+        __threadfence();
+        const unsigned ticket = atomicAdd(p.counter, 1u);
+        s_last = (ticket == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (MODE != MODE_GHASH && !active) {
+        fill_aes_tables<TPB>(sm, p.tab.te0);
+        __syncthreads();
+    }
+    uint4 acc = make_uint4(0, 0, 0, 0);
+    for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
+    acc = cta_xor_reduce(acc, red);
+    if (t == 0) {
+        // a10: length block BE64(8a) || BE64(8 len), one more multiply by H
+        const uint64_t abits = p.aad_len * 8, cbits = p.len * 8;
+        const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
+                                   bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
+        const uint4 S = gf_mul_mem(xor4(acc, L), __ldg(p.tab.h));
+        if (MODE == MODE_GHASH) {
+            *p.tag_out = S;
+        } else {
+            // a3 + a11: E_K(J0), J0 = IV || 0^31 || 1; tag; constant-time compare
+            const uint4 ek = aes_rounds<NR>(p, sm, lane4, p.iv_rk0[0], p.iv_rk0[1], p.iv_rk0[2], bswap32(1u) ^ p.rk[3]);
+            const uint4 tag = xor4(S, ek);
+            if (MODE == MODE_ENCRYPT) {
+                *p.tag_out = tag;
+            } else {
+                uint4 expect = make_uint4(p.tag_expect[0], p.tag_expect[1], p.tag_expect[2], p.tag_expect[3]);
+                if (p.tag_in != nullptr) expect = *p.tag_in;
+                const uint32_t diff = (tag.x ^ expect.x) | (tag.y ^ expect.y) | (tag.z ^ expect.z) | (tag.w ^ expect.w);
+                *p.status = diff != 0 ? 1 : 0;
+            }
+        }
+        *p.counter = 0;   // ready for the next launch on this context
+    }
+}
+
+// ---- host side ------------------------------------------------------------------------------------
+template <int NR, int MODE, int TPB>
+static cudaError_t launch_one(int blocks, const GcmParams &p, cudaStream_t s)
+{
+    static bool configured[64] = {false};   // per instantiation and device; the attribute is sticky
+    auto kern = gcm_fused_kernel<NR, MODE, TPB>;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FUSED_SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
+    }
+    kern<<<blocks, TPB, FUSED_SMEM_BYTES, s>>>(p);
+    return cudaGetLastError();
+}
+
+template <int TPB>
+static cudaError_t launch_tpb(int nr, int mode, int blocks, const GcmParams &p, cudaStream_t s)
+{
+    if (mode == MODE_GHASH) return launch_one<10, MODE_GHASH, TPB>(blocks, p, s);
+    if (nr == 10) return mode == MODE_ENCRYPT ? launch_one<10, MODE_ENCRYPT, TPB>(blocks, p, s)
+                                              : launch_one<10, MODE_DECRYPT, TPB>(blocks, p, s);
+    return mode == MODE_ENCRYPT ? launch_one<14, MODE_ENCRYPT, TPB>(blocks, p, s)
+                                : launch_one<14, MODE_DECRYPT, TPB>(blocks, p, s);
+}
+
+cudaError_t launch_fused(int nr, int mode, int threads, int blocks, const GcmParams &p, cudaStream_t s)
+{
+    if (threads == 256) return launch_tpb<256>(nr, mode, blocks, p, s);
+    return launch_tpb<512>(nr, mode, blocks, p, s);
+}

@@ -1,0 +1,309 @@
+"""ctypes binding of libb200gcm.so -- same names as include/gcm.h, marshalling only.
+
+Device buffers are torch uint8 CUDA tensors (PyTorch is used for device memory and streams only);
+anything exposing data_ptr()/numel() works, and plain ints are taken as raw device addresses.
+Every step of the path (key schedule, H powers, CTR, GHASH, tag, compare, wipe) runs in the
+library's CUDA kernels.  If the library is missing this module raises: there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Iterable, List, Optional, Sequence, Tuple
+
+GCM_OK, GCM_ERR_AUTH, GCM_ERR_ARG, GCM_ERR_LEN, GCM_ERR_CUDA, GCM_ERR_NOMEM = 0, 1, -1, -2, -3, -4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libb200gcm.so")
+
+EXPORTED_SYMBOLS = [
+    "gcm_version", "gcm_set_device", "gcm_last_cuda_error", "gcm_last_cuda_error_string",
+    "gcm_init", "gcm_destroy", "gcm_set_geometry", "gcm_get_geometry", "gcm_get_hash_subkey",
+    "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
+    "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
+]
+
+
+class GcmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        detail = ""
+        if code == GCM_ERR_CUDA:
+            detail = ": " + gcm_last_cuda_error_string()
+        super().__init__("%s failed with code %d%s" % (where, code, detail))
+
+
+class GcmMsg(ctypes.Structure):
+    """struct gcm_msg of include/gcm.h"""
+    _fields_ = [
+        ("key", ctypes.c_void_p),
+        ("key_bits", ctypes.c_int),
+        ("iv", ctypes.c_uint8 * 12),
+        ("d_aad", ctypes.c_void_p),
+        ("aad_len", ctypes.c_uint64),
+        ("d_in", ctypes.c_void_p),
+        ("len", ctypes.c_uint64),
+        ("d_out", ctypes.c_void_p),
+        ("tag", ctypes.c_uint8 * 16),
+        ("status", ctypes.c_int),
+    ]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            "libb200gcm.so is not built (%s). Run `python -m paper_2602_23067_b200.build` "
+            "(needs nvcc); there is no CPU fallback." % _LIB_PATH)
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, u64, ci = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int
+    L.gcm_version.restype = ctypes.c_char_p
+    L.gcm_version.argtypes = []
+    L.gcm_set_device.argtypes = [ci]
+    L.gcm_last_cuda_error.argtypes = []
+    L.gcm_last_cuda_error_string.restype = ctypes.c_char_p
+    L.gcm_last_cuda_error_string.argtypes = []
+    L.gcm_init.argtypes = [ctypes.POINTER(vp), ctypes.c_char_p, ci]
+    L.gcm_destroy.argtypes = [vp]
+    L.gcm_destroy.restype = None
+    L.gcm_set_geometry.argtypes = [vp, ci, ci]
+    L.gcm_get_geometry.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci)]
+    L.gcm_get_hash_subkey.argtypes = [vp, ctypes.c_char_p]
+    L.gcm_encrypt.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
+    L.gcm_decrypt_verify.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
+    L.gcm_encrypt_async.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, vp, vp]
+    L.gcm_decrypt_verify_async.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, vp, vp, vp]
+    L.gcm_ghash_async.argtypes = [vp, vp, u64, vp, u64, vp, vp]
+    L.gcm_encrypt_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
+    L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
+    L.gcm_batch_release.argtypes = []
+    L.gcm_batch_release.restype = None
+    return L
+
+
+_L = _load()
+
+
+# ---- marshalling ---------------------------------------------------------------------------------
+def _dev(buf) -> Tuple[Optional[int], int]:
+    """(device address or None, byte length) of a device buffer argument."""
+    if buf is None:
+        return None, 0
+    if isinstance(buf, int):
+        raise TypeError("raw device addresses need an explicit length; pass (ptr, nbytes)")
+    if isinstance(buf, tuple):
+        return (int(buf[0]) or None), int(buf[1])
+    if not getattr(buf, "is_cuda", False):
+        raise TypeError("device buffer expected (torch CUDA tensor)")
+    if not buf.is_contiguous():
+        raise ValueError("device buffer must be contiguous")
+    n = buf.numel() * buf.element_size()
+    return (buf.data_ptr() if n else None), n
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+def _check(rc: int, where: str, ok: Sequence[int] = (GCM_OK,)) -> int:
+    if rc not in ok:
+        raise GcmError(rc, where)
+    return rc
+
+
+# ---- the C ABI, one function per entry point -----------------------------------------------------
+def gcm_version() -> str:
+    return _L.gcm_version().decode()
+
+
+def gcm_set_device(ordinal: int) -> None:
+    _check(_L.gcm_set_device(int(ordinal)), "gcm_set_device")
+
+
+def gcm_last_cuda_error() -> int:
+    return _L.gcm_last_cuda_error()
+
+
+def gcm_last_cuda_error_string() -> str:
+    return _L.gcm_last_cuda_error_string().decode()
+
+
+def gcm_init(key: bytes, key_bits: Optional[int] = None) -> int:
+    key = bytes(key)
+    bits = 8 * len(key) if key_bits is None else int(key_bits)
+    h = ctypes.c_void_p()
+    _check(_L.gcm_init(ctypes.byref(h), key, bits), "gcm_init")
+    return h.value
+
+
+def gcm_destroy(ctx: Optional[int]) -> None:
+    if ctx:
+        _L.gcm_destroy(ctx)
+
+
+def gcm_set_geometry(ctx: int, grid: int = 0, threads: int = 0) -> None:
+    _check(_L.gcm_set_geometry(ctx, int(grid), int(threads)), "gcm_set_geometry")
+
+
+def gcm_get_geometry(ctx: int) -> Tuple[int, int]:
+    g, t = ctypes.c_int(), ctypes.c_int()
+    _check(_L.gcm_get_geometry(ctx, ctypes.byref(g), ctypes.byref(t)), "gcm_get_geometry")
+    return g.value, t.value
+
+
+def gcm_get_hash_subkey(ctx: int) -> bytes:
+    buf = ctypes.create_string_buffer(16)
+    _check(_L.gcm_get_hash_subkey(ctx, buf), "gcm_get_hash_subkey")
+    return buf.raw
+
+
+def gcm_encrypt(ctx: int, iv: bytes, aad, pt, ct, stream=None) -> bytes:
+    """Encrypts device buffer `pt` into device buffer `ct` (same size; may be the same tensor) and
+    returns the 16-byte tag."""
+    a_ptr, a_len = _dev(aad)
+    p_ptr, p_len = _dev(pt)
+    c_ptr, c_len = _dev(ct)
+    if c_len != p_len:
+        raise ValueError("ct and pt sizes differ")
+    tag = ctypes.create_string_buffer(16)
+    _check(_L.gcm_encrypt(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)), "gcm_encrypt")
+    return tag.raw
+
+
+def gcm_decrypt_verify(ctx: int, iv: bytes, aad, ct, pt, tag: bytes, stream=None) -> int:
+    """Returns GCM_OK (plaintext in `pt`) or GCM_ERR_AUTH (`pt` zero-filled)."""
+    a_ptr, a_len = _dev(aad)
+    c_ptr, c_len = _dev(ct)
+    p_ptr, p_len = _dev(pt)
+    if c_len != p_len:
+        raise ValueError("ct and pt sizes differ")
+    tag = bytes(tag)
+    if len(tag) != 16:
+        raise ValueError("tag must be 16 bytes")
+    return _check(_L.gcm_decrypt_verify(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
+                  "gcm_decrypt_verify", ok=(GCM_OK, GCM_ERR_AUTH))
+
+
+def gcm_encrypt_async(ctx: int, iv: bytes, aad, pt, ct, d_tag, stream=None) -> None:
+    a_ptr, a_len = _dev(aad)
+    p_ptr, p_len = _dev(pt)
+    c_ptr, _ = _dev(ct)
+    t_ptr, t_len = _dev(d_tag)
+    if t_len < 16:
+        raise ValueError("d_tag must hold 16 bytes")
+    _check(_L.gcm_encrypt_async(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, t_ptr, _stream(stream)),
+           "gcm_encrypt_async")
+
+
+def gcm_decrypt_verify_async(ctx: int, iv: bytes, aad, ct, pt, d_tag, d_status, stream=None) -> None:
+    a_ptr, a_len = _dev(aad)
+    c_ptr, c_len = _dev(ct)
+    p_ptr, _ = _dev(pt)
+    t_ptr, t_len = _dev(d_tag)
+    s_ptr, s_len = _dev(d_status)
+    if t_len < 16 or s_len < 4:
+        raise ValueError("d_tag must hold 16 bytes and d_status 4")
+    _check(_L.gcm_decrypt_verify_async(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, t_ptr, s_ptr,
+                                       _stream(stream)), "gcm_decrypt_verify_async")
+
+
+def gcm_ghash_async(ctx: int, aad, c, d_out, stream=None) -> None:
+    a_ptr, a_len = _dev(aad)
+    c_ptr, c_len = _dev(c)
+    o_ptr, o_len = _dev(d_out)
+    if o_len < 16:
+        raise ValueError("d_out must hold 16 bytes")
+    _check(_L.gcm_ghash_async(ctx, a_ptr, a_len, c_ptr, c_len, o_ptr, _stream(stream)), "gcm_ghash_async")
+
+
+def _pack_msgs(msgs: Iterable[dict], decrypt: bool):
+    msgs = list(msgs)
+    arr = (GcmMsg * max(1, len(msgs)))()
+    keep = []
+    for i, m in enumerate(msgs):
+        key = ctypes.create_string_buffer(bytes(m["key"]), len(m["key"]))
+        keep.append(key)
+        arr[i].key = ctypes.cast(key, ctypes.c_void_p)
+        arr[i].key_bits = 8 * len(m["key"])
+        arr[i].iv[:] = list(bytes(m["iv"]))
+        a_ptr, a_len = _dev(m.get("aad"))
+        i_ptr, i_len = _dev(m["input"])
+        o_ptr, o_len = _dev(m["output"])
+        if o_len != i_len:
+            raise ValueError("message %d: input and output sizes differ" % i)
+        arr[i].d_aad, arr[i].aad_len = a_ptr, a_len
+        arr[i].d_in, arr[i].len = i_ptr, i_len
+        arr[i].d_out = o_ptr
+        if decrypt:
+            arr[i].tag[:] = list(bytes(m["tag"]))
+    return arr, len(msgs), keep
+
+
+def gcm_encrypt_batch(msgs: Iterable[dict], stream=None) -> List[bytes]:
+    """msgs: dicts with key, iv, aad (device or None), input, output (device).  Returns the tags."""
+    arr, n, keep = _pack_msgs(msgs, decrypt=False)
+    _check(_L.gcm_encrypt_batch(arr, n, _stream(stream)), "gcm_encrypt_batch")
+    del keep
+    return [bytes(arr[i].tag) for i in range(n)]
+
+
+def gcm_decrypt_verify_batch(msgs: Iterable[dict], stream=None) -> List[int]:
+    """msgs as above plus `tag`.  Returns the per-message status list (GCM_OK / GCM_ERR_AUTH)."""
+    arr, n, keep = _pack_msgs(msgs, decrypt=True)
+    rc = _L.gcm_decrypt_verify_batch(arr, n, _stream(stream))
+    if rc < 0:
+        raise GcmError(rc, "gcm_decrypt_verify_batch")
+    del keep
+    return [arr[i].status for i in range(n)]
+
+
+def gcm_batch_release() -> None:
+    _L.gcm_batch_release()
+
+
+class Context:
+    """Owns one gcm_ctx.  Convenience wrapper over the functions above."""
+
+    def __init__(self, key: bytes):
+        self.handle = gcm_init(key)
+        self.key_bits = 8 * len(key)
+
+    def close(self) -> None:
+        if self.handle:
+            gcm_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_geometry(self, grid: int = 0, threads: int = 0) -> None:
+        gcm_set_geometry(self.handle, grid, threads)
+
+    def encrypt(self, iv, aad, pt, ct=None, stream=None):
+        import torch
+        if ct is None:
+            ct = torch.empty_like(pt)
+        return ct, gcm_encrypt(self.handle, iv, aad, pt, ct, stream)
+
+    def decrypt_verify(self, iv, aad, ct, tag, pt=None, stream=None):
+        import torch
+        if pt is None:
+            pt = torch.empty_like(ct)
+        return gcm_decrypt_verify(self.handle, iv, aad, ct, pt, tag, stream), pt

@@ -1,0 +1,62 @@
+"""The C-ABI library loads and exports every symbol include/gcm.h declares (no compute calls: no GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib_path():
+    from paper_2602_23067_b200 import build
+    return build.build()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "gcm.h")).read()
+    return sorted(set(re.findall(r"GCM_API\s+[\w \*]+?\b(gcm_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_boundary():
+    names = declared_symbols()
+    for must in ("gcm_init", "gcm_destroy", "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_batch",
+                 "gcm_decrypt_verify_batch", "gcm_encrypt_async", "gcm_decrypt_verify_async"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(lib_path):
+    L = ctypes.CDLL(lib_path)
+    for name in declared_symbols():
+        assert hasattr(L, name), name
+    L.gcm_version.restype = ctypes.c_char_p
+    assert b"sm_100a" in L.gcm_version()
+
+
+def test_binding_lists_the_same_symbols(lib_path):
+    import paper_2602_23067_b200 as pkg
+    assert sorted(pkg.EXPORTED_SYMBOLS) == declared_symbols()
+    assert pkg.library_path() == lib_path
+
+
+def test_argument_errors_without_gpu(lib_path):
+    """Argument validation happens before any CUDA call."""
+    import paper_2602_23067_b200 as pkg
+    with pytest.raises(pkg.GcmError) as e:
+        pkg.gcm_init(bytes(24))            # AES-192 is outside reading S1
+    assert e.value.code == pkg.GCM_ERR_ARG
+    L = ctypes.CDLL(lib_path)
+    assert L.gcm_init(None, b"0" * 16, 128) == pkg.GCM_ERR_ARG
+    assert L.gcm_encrypt(None, None, None, 0, None, 0, None, None, None) == pkg.GCM_ERR_ARG
+
+
+def test_no_cpu_fallback_in_product_path():
+    """The product package never imports the oracle (checked textually)."""
+    pkg_dir = os.path.join(ROOT, "paper_2602_23067_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text, f
+                assert "liboracle" not in text, f

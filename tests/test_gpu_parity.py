@@ -1,0 +1,298 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, bit-exact.
+
+Integer / byte work only: the bar is equality of every ciphertext byte and every tag byte.
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def G():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2602_23067_b200 as pkg
+    return pkg
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rnd(rng, n):
+    return rng.integers(0, 256, n, dtype=np.uint8)
+
+
+def check_message(G, oracle, ctx, key, iv, aad, pt, note=""):
+    d_aad = dev(aad) if len(aad) else None
+    d_pt = dev(pt)
+    d_ct = torch.empty_like(d_pt)
+    tag = G.gcm_encrypt(ctx, iv, d_aad, d_pt, d_ct)
+    ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+    got = d_ct.cpu().numpy()
+    assert np.array_equal(got, ref_ct), "ciphertext mismatch %s" % note
+    assert tag == ref_tag, "tag mismatch %s" % note
+    d_back = torch.empty_like(d_pt)
+    rc = G.gcm_decrypt_verify(ctx, iv, d_aad, d_ct, d_back, tag)
+    assert rc == G.GCM_OK, note
+    assert np.array_equal(d_back.cpu().numpy(), np.asarray(pt)), "roundtrip %s" % note
+    return d_aad, d_ct, tag
+
+
+@pytest.mark.parametrize("klen", [16, 32])
+def test_setup_kernel_hash_subkey(G, oracle, klen):
+    rng = np.random.default_rng(9000 + klen)
+    for _ in range(3):
+        key = rnd(rng, klen).tobytes()
+        ctx = G.gcm_init(key)
+        try:
+            assert G.gcm_get_hash_subkey(ctx) == oracle.hash_subkey(key)
+        finally:
+            G.gcm_destroy(ctx)
+
+
+@pytest.mark.parametrize("klen", [16, 32])
+def test_small_lengths_default_geometry(G, oracle, klen):
+    rng = np.random.default_rng(9100 + klen)
+    key = rnd(rng, klen).tobytes()
+    ctx = G.gcm_init(key)
+    try:
+        sizes = [(0, 0), (0, 1), (0, 16), (0, 2880), (1, 0), (15, 0), (16, 0), (17, 5), (31, 16), (32, 17),
+                 (100, 40), (8191, 0), (8192, 0), (8193, 16), (8192 - 16, 16), (8192 * 3 + 7, 2880),
+                 (65536, 256), (100003, 33)]
+        for (n, a) in sizes:
+            iv = rnd(rng, 12).tobytes()
+            check_message(G, oracle, ctx, key, iv, rnd(rng, a), rnd(rng, n), "len=%d aad=%d" % (n, a))
+    finally:
+        G.gcm_destroy(ctx)
+
+
+@pytest.mark.parametrize("klen", [16, 32])
+def test_geometry_agnostic(G, oracle, klen):
+    """the result never depends on the launch geometry.  Small grids force
+    long per-thread chains, ragged last rows and every CTA-correction exponent."""
+    rng = np.random.default_rng(9200 + klen)
+    key = rnd(rng, klen).tobytes()
+    iv = rnd(rng, 12).tobytes()
+    aad = rnd(rng, 2880)
+    pt = rnd(rng, 16 * 512 * 11 + 16 * 77 + 5)
+    ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+    ctx = G.gcm_init(key)
+    try:
+        d_aad, d_pt = dev(aad), dev(pt)
+        for (grid, threads) in [(1, 512), (1, 256), (2, 512), (3, 256), (5, 512), (7, 256), (148, 512),
+                                (148, 256), (200, 512), (0, 0)]:
+            G.gcm_set_geometry(ctx, grid, threads)
+            d_ct = torch.empty_like(d_pt)
+            tag = G.gcm_encrypt(ctx, iv, d_aad, d_pt, d_ct)
+            assert np.array_equal(d_ct.cpu().numpy(), ref_ct), (grid, threads)
+            assert tag == ref_tag, (grid, threads)
+            d_back = torch.empty_like(d_pt)
+            assert G.gcm_decrypt_verify(ctx, iv, d_aad, d_ct, d_back, tag) == G.GCM_OK
+            assert np.array_equal(d_back.cpu().numpy(), pt)
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_many_lengths_small_geometry(G, oracle):
+    """Every length 0..700 bytes region and block counts around row boundaries with grid=2, 256
+    threads, so rows, pads and tails of every shape occur."""
+    rng = np.random.default_rng(9300)
+    key = rnd(rng, 16).tobytes()
+    ctx = G.gcm_init(key)
+    try:
+        G.gcm_set_geometry(ctx, 2, 256)
+        lens = list(range(0, 70)) + [16 * 255, 16 * 256 - 1, 16 * 256, 16 * 256 + 1, 16 * 257, 16 * 511 + 3,
+                                       16 * 512, 16 * 513 - 15, 16 * 1024, 16 * 1025 + 9, 16 * 2047, 16 * 2049]
+        for n in lens:
+            for a in (0, 7, 16, 100):
+                iv = rnd(rng, 12).tobytes()
+                check_message(G, oracle, ctx, key, iv, rnd(rng, a), rnd(rng, n), "len=%d aad=%d" % (n, a))
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_in_place_and_unaligned(G, oracle):
+    rng = np.random.default_rng(9400)
+    key = rnd(rng, 32).tobytes()
+    iv = rnd(rng, 12).tobytes()
+    aad = rnd(rng, 50)
+    n = 16 * 512 * 3 + 100
+    pt = rnd(rng, n)
+    ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+    ctx = G.gcm_init(key)
+    try:
+        d_aad = dev(aad)
+        buf = dev(pt).clone()
+        tag = G.gcm_encrypt(ctx, iv, d_aad, buf, buf)          # in place
+        assert tag == ref_tag and np.array_equal(buf.cpu().numpy(), ref_ct)
+        assert G.gcm_decrypt_verify(ctx, iv, d_aad, buf, buf, tag) == G.GCM_OK
+        assert np.array_equal(buf.cpu().numpy(), pt)
+        for (oi, oo, oa) in [(1, 0, 0), (0, 3, 0), (5, 5, 1), (15, 9, 7)]:
+            big_in = torch.zeros(n + 64, dtype=torch.uint8, device="cuda")
+            big_out = torch.zeros(n + 64, dtype=torch.uint8, device="cuda")
+            big_aad = torch.zeros(len(aad) + 16, dtype=torch.uint8, device="cuda")
+            big_in[oi: oi + n] = dev(pt)
+            big_aad[oa: oa + len(aad)] = d_aad
+            tag = G.gcm_encrypt(ctx, iv, big_aad[oa: oa + len(aad)], big_in[oi: oi + n], big_out[oo: oo + n])
+            out = big_out.cpu().numpy()
+            assert tag == ref_tag, (oi, oo, oa)
+            assert np.array_equal(out[oo: oo + n], ref_ct), (oi, oo, oa)
+            assert not out[:oo].any() and not out[oo + n:].any(), "wrote outside the output range"
+        # partial overlap is refused
+        big = torch.zeros(n + 64, dtype=torch.uint8, device="cuda")
+        with pytest.raises(G.GcmError) as e:
+            G.gcm_encrypt(ctx, iv, d_aad, big[0:n], big[16: 16 + n])
+        assert e.value.code == G.GCM_ERR_ARG
+    finally:
+        G.gcm_destroy(ctx)
+
+
+@pytest.mark.parametrize("klen", [16, 32])
+def test_tamper_detection_and_suppression(G, oracle, klen):
+    """PAPER.md L219 (validation gate), L243 (payload zero-filled), L157 (AAD binding)."""
+    rng = np.random.default_rng(9500 + klen)
+    key = rnd(rng, klen).tobytes()
+    iv = rnd(rng, 12).tobytes()
+    aad = rnd(rng, 2880)
+    pt = rnd(rng, 16 * 512 * 2 + 33)
+    ctx = G.gcm_init(key)
+    try:
+        d_aad, d_ct, tag = check_message(G, oracle, ctx, key, iv, aad, pt)
+        n = len(pt)
+
+        def rejected(iv_=iv, aad_=d_aad, ct_=d_ct, tag_=tag):
+            out = torch.full((ct_.numel(),), 0xAA, dtype=torch.uint8, device="cuda")
+            rc = G.gcm_decrypt_verify(ctx, iv_, aad_, ct_, out, tag_)
+            return rc == G.GCM_ERR_AUTH and not bool(out.any().item())
+
+        for pos in (0, n // 2, n - 1):
+            bad = d_ct.clone(); bad[pos] ^= 0x04
+            assert rejected(ct_=bad)
+        for bit in (0, 63, 127):
+            t = bytearray(tag); t[bit // 8] ^= 1 << (bit % 8)
+            assert rejected(tag_=bytes(t))
+        bad_aad = d_aad.clone(); bad_aad[100] ^= 1
+        assert rejected(aad_=bad_aad)
+        assert rejected(aad_=d_aad[:-1].clone())
+        v = bytearray(iv); v[11] ^= 1
+        assert rejected(iv_=bytes(v))
+        assert rejected(ct_=d_ct[:-1].clone())
+        # the oracle agrees on rejection and on zeros
+        bad = d_ct.clone(); bad[7] ^= 0x80
+        rc, out = oracle.gcm_decrypt_verify(key, iv, aad, bad.cpu().numpy(), tag)
+        assert rc == oracle.AUTH_FAIL and not out.any()
+        # async form: status word + wipe kernel on the stream
+        d_tag = dev(np.frombuffer(tag, np.uint8))
+        d_status = torch.full((1,), -7, dtype=torch.int32, device="cuda")
+        out = torch.full((n,), 0x55, dtype=torch.uint8, device="cuda")
+        G.gcm_decrypt_verify_async(ctx, iv, d_aad, bad, out, d_tag, d_status)
+        torch.cuda.synchronize()
+        assert int(d_status.item()) == G.GCM_ERR_AUTH and not bool(out.any().item())
+        G.gcm_decrypt_verify_async(ctx, iv, d_aad, d_ct, out, d_tag, d_status)
+        torch.cuda.synchronize()
+        assert int(d_status.item()) == G.GCM_OK and np.array_equal(out.cpu().numpy(), pt)
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_async_encrypt_and_ghash_only(G, oracle):
+    rng = np.random.default_rng(9600)
+    key = rnd(rng, 32).tobytes()
+    iv = rnd(rng, 12).tobytes()
+    aad = rnd(rng, 77)
+    pt = rnd(rng, 16 * 512 * 5 + 9)
+    ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+    ctx = G.gcm_init(key)
+    try:
+        d_aad, d_pt = dev(aad), dev(pt)
+        d_ct = torch.empty_like(d_pt)
+        d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        G.gcm_encrypt_async(ctx, iv, d_aad, d_pt, d_ct, d_tag)
+        torch.cuda.synchronize()
+        assert np.array_equal(d_ct.cpu().numpy(), ref_ct)
+        assert d_tag.cpu().numpy().tobytes() == ref_tag
+        d_s = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        G.gcm_ghash_async(ctx, d_aad, d_ct, d_s)
+        torch.cuda.synchronize()
+        assert d_s.cpu().numpy().tobytes() == oracle.ghash(oracle.hash_subkey(key), aad, ref_ct)
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_error_codes(G):
+    ctx = G.gcm_init(bytes(16))
+    try:
+        t = torch.zeros(32, dtype=torch.uint8, device="cuda")
+        import ctypes
+        from paper_2602_23067_b200 import gcm as B
+        tag = ctypes.create_string_buffer(16)
+        # length limit
+        assert B._L.gcm_encrypt(ctx, bytes(12), None, 0, t.data_ptr(), (1 << 36) - 31, t.data_ptr(), tag, None) == G.GCM_ERR_LEN
+        # NULL data with non-zero length
+        assert B._L.gcm_encrypt(ctx, bytes(12), None, 5, t.data_ptr(), 16, t.data_ptr(), tag, None) == G.GCM_ERR_ARG
+        assert B._L.gcm_encrypt(ctx, None, None, 0, t.data_ptr(), 16, t.data_ptr(), tag, None) == G.GCM_ERR_ARG
+        with pytest.raises(G.GcmError):
+            G.gcm_set_geometry(ctx, 5, 100)
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_config_c1_full(G, oracle):
+    m = workloads.config_c1()
+    ctx = G.gcm_init(m.key)
+    try:
+        check_message(G, oracle, ctx, m.key, m.iv, m.aad, m.payload, "C1")
+    finally:
+        G.gcm_destroy(ctx)
+
+
+def test_config_c3_scaled_batch(G, oracle):
+    msgs = workloads.config_c3(n_images=4, ny=512, nx=384, n_sources=20)
+    batch = []
+    for m in msgs:
+        d_in = dev(m.payload)
+        batch.append({"key": m.key, "iv": m.iv, "aad": dev(m.aad), "input": d_in, "output": torch.empty_like(d_in)})
+    tags = G.gcm_encrypt_batch(batch)
+    for m, b, tag in zip(msgs, batch, tags):
+        ref_ct, ref_tag = oracle.gcm_encrypt(m.key, m.iv, m.aad, m.payload)
+        assert tag == ref_tag, m.name
+        assert np.array_equal(b["output"].cpu().numpy(), ref_ct), m.name
+    # structured plaintext must still look like noise: no repeated ciphertext block
+    ct0 = batch[0]["output"].cpu().numpy()
+    blocks = ct0[: ct0.size // 16 * 16].reshape(-1, 16)
+    assert len({bytes(b) for b in blocks[:20000]}) == min(20000, len(blocks))
+    dec = []
+    for b, tag in zip(batch, tags):
+        dec.append({"key": b["key"], "iv": b["iv"], "aad": b["aad"], "input": b["output"],
+                    "output": torch.empty_like(b["output"]), "tag": tag})
+    dec[2]["tag"] = bytes(16)
+    st = G.gcm_decrypt_verify_batch(dec)
+    assert st == [G.GCM_OK, G.GCM_OK, G.GCM_ERR_AUTH, G.GCM_OK]
+    for i, (m, d) in enumerate(zip(msgs, dec)):
+        got = d["output"].cpu().numpy()
+        if i == 2:
+            assert not got.any()
+        else:
+            assert np.array_equal(got, m.payload)
+    G.gcm_batch_release()
+
+
+def test_config_c4_scaled_batch(G, oracle):
+    msgs = workloads.config_c4(n_messages=60, max_len=20000)
+    batch = []
+    for m in msgs:
+        d_in = dev(m.payload)
+        batch.append({"key": m.key, "iv": m.iv, "aad": dev(m.aad) if m.aad.size else None,
+                      "input": d_in, "output": torch.empty_like(d_in)})
+    tags = G.gcm_encrypt_batch(batch)
+    for m, b, tag in zip(msgs, batch, tags):
+        ref_ct, ref_tag = oracle.gcm_encrypt(m.key, m.iv, m.aad, m.payload)
+        assert tag == ref_tag, m.name
+        assert np.array_equal(b["output"].cpu().numpy(), ref_ct), m.name
+    G.gcm_batch_release()
