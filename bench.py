@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- AES-256-GCM encrypt GB/s on a 4 GiB message (BASELINE.json config 5), device-timed.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--size-mib M]
+
+One "step" = one pass of the whole hot path (counters, AES rounds, payload
+XOR, GHASH fold + combine, tag) over one 4 GiB synthetic message that is already resident in HBM.
+Prints ONE JSON line (rank 0).  With N > 1 (torchrun) every rank encrypts its own message on its
+own GPU: messages are independent, there is no data-path collective ("scaling": "weak"); NCCL is
+used only for the barrier and the max-over-ranks of the device time.
+
+  value      payload GB/s (1e9 bytes), all ranks' bytes / max-over-ranks device time of the K steps
+  e2e        same metric through gcm_encrypt_host(): pinned HOST buffers in and out, the H2D and D2H
+             copies inside the timed region
+  roofline   achieved payload GB/s of the fused kernel vs the shared-memory-pipe bound derived in
+             DESIGN.md section 6 (the binding unit; the HBM figure is reported beside it)
+  cpu_baseline  the CPU oracle, as it stands, on the host cores, on a bounded sample of the workload
+
+--impl reference times the oracle itself (this tier has no reference implementation to install).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "AES-256-GCM encrypt GB/s (device-timed, 4 GiB msg)"
+UNIT = "GB/s"
+WORKLOAD = "C5: AES-256-GCM encrypt, one 4 GiB uniform-random message, 2880-byte FITS header AAD, 96-bit IV"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size-mib", type=float, default=4096.0, help="payload MiB (default: the 4 GiB of config 5)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-mib", type=float, default=48.0)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1])); mx.append(float(f[2])); power.append(float(f[3]))
+                except ValueError:
+                    continue
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            # samples under load: the upper half (idle samples before/after the region sit at low clocks)
+            load = sorted(sm)[len(sm) // 2:]
+            out.update(sm_mhz=statistics.median(load), sm_max_mhz=max(mx), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=max(power) if power else None)
+        return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# roofline
+# ---------------------------------------------------------------------------------------------------
+def measured_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
+
+
+def pipe_bound_gbs(nr: int, sm_count: int, sm_mhz: float) -> dict:
+    """Shared-memory-pipe bound of the method: per 16-byte block the path needs
+    16*nr - 12 conflict-free 4-byte table reads (the 12 first-round reads of the constant IV columns
+    are hoisted) and 16 16-byte GHASH table reads = 64 bank-lanes; an SM serves 32 bank-lanes (one
+    128-byte wavefront) per cycle."""
+    lanes = 16 * nr - 12 + 64
+    cycles = lanes / 32.0
+    return {"lanes_per_block": lanes, "cycles_per_block_per_sm": cycles,
+            "gbs": sm_count * sm_mhz * 1e6 * 16.0 / cycles / 1e9}
+
+
+def traffic_per_launch(payload_bytes: int):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/), scaled by size."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        d = json.load(open(p))
+        return d["dram_bytes_per_payload_byte"] * payload_bytes
+    except Exception:
+        return None
+
+
+# ---------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline of our arm, and the whole --impl reference arm)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample_gbs(sample_bytes: int):
+    """AES-256-GCM encrypt of a `sample_bytes` prefix-sized message of the same recipe on the host
+    cores: CTR chunked over all cores, GHASH the sequential Horner chain on one (oracle as it stands)."""
+    import numpy as np
+    from oracle import oracle as O
+    import workloads
+    cores = os.cpu_count() or 1
+    m = workloads.config_c5(payload_bytes=sample_bytes)
+    O.lib()
+    t0 = time.perf_counter()
+    ct, tag = O.gcm_encrypt_threaded(m.key, m.iv, m.aad, m.payload, threads=cores, segment_blocks=0)
+    dt = time.perf_counter() - t0
+    assert ct.size == sample_bytes and len(tag) == 16
+    return sample_bytes / dt / 1e9, cores, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sample = int(min(args.cpu_sample_mib, 16.0) * (1 << 20))
+    steps, warm = max(1, min(args.steps, 5)), max(0, min(args.warmup, 1))
+    for _ in range(warm):
+        oracle_sample_gbs(sample)
+    t0 = time.perf_counter()
+    cores = 1
+    for _ in range(steps):
+        _, cores, _ = oracle_sample_gbs(sample)
+    dt = time.perf_counter() - t0
+    gbs = steps * sample / dt / 1e9
+    sample_txt = "first %.0f MiB-sized message of the C5 recipe per step (the 4 GiB message would take minutes)" % (sample / 2 ** 20)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample_txt},
+        "cpu_baseline": {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_txt},
+        "e2e": {"value": gbs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2602_23067_b200 as G
+    import workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    G.gcm_set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    n = int(args.size_mib * (1 << 20))
+    m = workloads.config_c5(payload_bytes=n, with_payload=False)
+    key = bytes(x ^ rank for x in m.key) if rank else m.key      # one independent message per rank
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(workloads.SEEDS["C5"] + rank)
+    # uniform random bytes, generated on the device 8 bytes at a time
+    pt = torch.randint(-2 ** 63, 2 ** 63 - 1, ((n + 7) // 8,), dtype=torch.int64, device="cuda", generator=gen).view(torch.uint8)[:n]
+    ct = torch.empty(n, dtype=torch.uint8, device="cuda")
+    aad = torch.from_numpy(m.aad).cuda()
+    d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    ctx = G.gcm_init(key)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+
+    # sampled parity check outside the timed region (oracle computes single keystream blocks)
+    verified = 0
+    if rank == 0:
+        from oracle import oracle as O
+        rs = np.random.default_rng(5)
+        nblk = n // 16
+        for g in sorted({0, nblk - 1, *rs.integers(0, max(1, nblk), 6).tolist()}):
+            ks = np.frombuffer(O.keystream_block(key, m.iv, int(g)), np.uint8)
+            got = ct[16 * g: 16 * g + 16].cpu().numpy() ^ pt[16 * g: 16 * g + 16].cpu().numpy()
+            assert np.array_equal(got, ks), "keystream block %d differs from the oracle" % g
+            verified += 1
+
+    sampler = ClockSampler(local)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    torch.cuda.synchronize()
+    if rank == 0:
+        sampler.start()
+    ev[0].record(stream)
+    for i in range(args.steps):
+        step()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else {}
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = world * args.steps * n / (total_ms * 1e-3) / 1e9
+
+    # end to end: pinned host buffers through gcm_encrypt_host (H2D + kernels + D2H inside the region)
+    e2e = None
+    if not args.no_e2e:
+        h_pt = torch.empty(n, dtype=torch.uint8).pin_memory()
+        h_ct = torch.empty(n, dtype=torch.uint8).pin_memory()
+        h_pt.copy_(pt)
+        h_aad = m.aad
+        G.gcm_encrypt_host(ctx, m.iv, h_aad, h_pt, h_ct, stream)          # warm-up (allocates staging)
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            tag_h = G.gcm_encrypt_host(ctx, m.iv, h_aad, h_pt, h_ct, stream)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        assert tag_h == d_tag.cpu().numpy().tobytes(), "host-path tag differs from device-path tag"
+        assert torch.equal(h_ct[:4096], ct[:4096].cpu()) and torch.equal(h_ct[-4096:], ct[-4096:].cpu())
+        e2e = {"value": world * args.e2e_steps * n / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": n + int(m.aad.size), "d2h_bytes_per_step": n + 16,
+               "steps": args.e2e_steps, "how": "gcm_encrypt_host: pinned host in/out, chunked H2D -> fused kernel -> D2H"}
+        del h_pt, h_ct
+
+    G.gcm_destroy(ctx)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    kernel_ms = statistics.mean(per)
+    achieved = n / (kernel_ms * 1e-3) / 1e9
+    pb = pipe_bound_gbs(14, sm_count, float(peaks.get("sm_max_mhz", 1965.0)))
+    hbm_peak = float(peaks["hbm_gbs"])
+    roofline = {
+        "bound": "alu", "pipe": "shared-memory wavefronts (LSU): %d bank-lanes per 16-byte block, 32 per SM-cycle" % pb["lanes_per_block"],
+        "achieved": achieved, "peak": pb["gbs"], "unit": UNIT, "frac": achieved / pb["gbs"],
+        "peak_source": "derived (DESIGN.md section 6): %d SMs x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s) x 16 B / %.3f cycles"
+                       % (sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks["_source"], pb["cycles_per_block_per_sm"]),
+        "traffic": traffic_per_launch(n),
+        "algorithmic_bytes_per_launch": 2 * n,
+        "hbm": {"achieved": 2 * achieved, "peak": hbm_peak, "unit": "GB/s", "frac": 2 * achieved / hbm_peak,
+                "of": peaks["_source"]},
+        "kernel": "gcm_fused_kernel<14, ENCRYPT, 512>", "kernel_ms_mean": kernel_ms,
+        "kernel_ms_median": statistics.median(per),
+    }
+    if clocks.get("sm_mhz"):
+        roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs(14, sm_count, clocks["sm_mhz"])["gbs"]
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        sample = int(args.cpu_sample_mib * (1 << 20))
+        gbs, cores, dt = oracle_sample_gbs(sample)
+        cpu = {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": "a %.0f MiB message of the same recipe (AES-256, 2880-byte AAD): CTR chunked over %d threads, "
+                         "GHASH sequential Horner on one" % (sample / 2 ** 20, cores)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": WORKLOAD if n == 4 << 30 else WORKLOAD + " [payload overridden: %d bytes]" % n,
+                   "payload_bytes": n, "aad_bytes": int(m.aad.size), "key_bits": 256,
+                   "l2": "inputs (4 GiB in + 4 GiB out per step) are larger than the 126 MB L2; no flush needed",
+                   "parallelism": "one independent message per GPU, no collective" if world > 1 else "single GPU",
+                   "verified_keystream_blocks_vs_oracle": verified},
+        "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
+        "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu,
+        "ms_per_step_median": statistics.median(per), "ms_per_step_std": statistics.pstdev(per),
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

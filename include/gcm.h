@@ -139,6 +139,25 @@ GCM_API int gcm_decrypt_verify_async(gcm_ctx *ctx, const uint8_t iv[12],
                              void *d_pt, const void *d_tag, void *d_status, void *cuda_stream);
 
 /*
+ * Host-buffer forms (the paper's data plane stages files through pinned host memory and overlaps
+ * the transfers with the kernels on CUDA streams): `h_*` are HOST
+ * pointers (pinned memory gives full PCIe rate; pageable memory works).  The message is cut into
+ * 64 MiB chunks that travel H2D -> fused kernel -> D2H on three internal streams; the running
+ * GHASH state is handed from chunk to chunk on the device.  Work already queued on `cuda_stream`
+ * is waited for; the call returns when the output and the tag / verdict are in host memory.
+ * On GCM_ERR_AUTH h_pt[0..len) is zero-filled.  aad_len < 2^32 here.
+ */
+GCM_API int gcm_encrypt_host(gcm_ctx *ctx, const uint8_t iv[12],
+                     const void *h_aad, uint64_t aad_len,
+                     const void *h_pt, uint64_t len,
+                     void *h_ct, uint8_t tag[16], void *cuda_stream);
+
+GCM_API int gcm_decrypt_verify_host(gcm_ctx *ctx, const uint8_t iv[12],
+                            const void *h_aad, uint64_t aad_len,
+                            const void *h_ct, uint64_t len,
+                            void *h_pt, const uint8_t tag[16], void *cuda_stream);
+
+/*
  * GHASH only (GMAC-style measurement; the paper's Table 5 "GHashKernelOnly",
  * PAPER.md L363, L379-L392): S = GHASH_H(A || 0* || C || 0* || len64(A) || len64(C)) over
  * device-resident data, 16 bytes written to d_out (device).  No AES on the payload.

@@ -10,6 +10,7 @@ from .gcm import (  # noqa: F401
     gcm_version, gcm_set_device, gcm_last_cuda_error, gcm_last_cuda_error_string,
     gcm_init, gcm_destroy, gcm_set_geometry, gcm_get_geometry, gcm_get_hash_subkey,
     gcm_encrypt, gcm_decrypt_verify, gcm_encrypt_async, gcm_decrypt_verify_async, gcm_ghash_async,
+    gcm_encrypt_host, gcm_decrypt_verify_host,
     gcm_encrypt_batch, gcm_decrypt_verify_batch, gcm_batch_release,
     library_path, EXPORTED_SYMBOLS,
 )

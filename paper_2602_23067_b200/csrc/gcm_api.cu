@@ -130,6 +130,7 @@ extern "C" void gcm_destroy(gcm_ctx *c)
 {
     if (!c) return;
     cudaSetDevice(c->device);
+    gcm_host_pipe_free(c);
     if (c->d_slab) {
         launch_wipe(c->d_slab, c->slab_bytes, nullptr, 0);
         cudaDeviceSynchronize();
@@ -178,7 +179,7 @@ extern "C" int gcm_get_hash_subkey(const gcm_ctx *c, uint8_t h[16])
 }
 
 // Argument checks and launch parameters common to encrypt / decrypt / ghash.
-static int build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
+int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
                         const void *d_in, uint64_t len, void *d_out, GcmParams *p, int *blocks)
 {
     if (!c) return GCM_ERR_ARG;
@@ -200,6 +201,8 @@ static int build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_a
     p->aad = (const uint8_t *)d_aad;
     p->len = len;
     p->aad_len = aad_len;
+    p->final_len = len;
+    p->final_aad_len = aad_len;
     p->n_full = len / 16;
     const uint64_t n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
     const uint64_t T = (uint64_t)c->threads;
@@ -237,7 +240,7 @@ extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d
     GcmParams p;
     int blocks = 0;
     if (!d_tag) return GCM_ERR_ARG;
-    int rc = build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_tag;
     CU(cudaSetDevice(c->device));
@@ -254,7 +257,7 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
     GcmParams p;
     int blocks = 0;
     if (!d_tag || !d_status) return GCM_ERR_ARG;
-    int rc = build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_in = (const uint4 *)d_tag;
     p.status = (int *)d_status;
@@ -274,7 +277,7 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     GcmParams p;
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
-    int rc = build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_out;
     CU(cudaSetDevice(c->device));
@@ -302,7 +305,7 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
     if (!c || !tag) return GCM_ERR_ARG;
     GcmParams p;
     int blocks = 0;
-    int rc = build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
     if (rc != GCM_OK) return rc;
     memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
     CU(cudaSetDevice(c->device));

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+struct HostPipe;          // gcm_host.cu: staging buffers, streams and events of the host-buffer entry points
+
 struct gcm_ctx {
     int device;
     int key_bits;
@@ -26,6 +28,11 @@ struct gcm_ctx {
     // host state
     uint32_t  h_rk[60];   // round keys (little-endian column words) for the kernel parameter block
     uint8_t  *h_pinned;   // 64 bytes of pinned memory: tag [0,16), status [16,20)
+    HostPipe *pipe;       // lazily created by gcm_encrypt_host / gcm_decrypt_verify_host
 };
 
 int gcm_cuda_fail(cudaError_t e);
+struct GcmParams;
+int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
+                     const void *d_in, uint64_t len, void *d_out, GcmParams *p, int *blocks);
+void gcm_host_pipe_free(gcm_ctx *c);

@@ -64,4 +64,13 @@ struct GcmParams {
     const uint4 *tag_in;     // device, 16 bytes or NULL -> tag_expect below
     uint32_t tag_expect[4];
     int      *status;        // device
+    // chunked (host-pipeline) operation: this launch covers payload blocks [ctr_base, ...) of a longer
+    // message.  chain_in/chain_pow: running GHASH state before this chunk and H^(GHASH blocks of this
+    // chunk); chain_out != NULL: store the new running state instead of finishing the tag.
+    uint32_t ctr_base;
+    const uint4 *chain_in;
+    const uint4 *chain_pow;
+    uint4    *chain_out;
+    uint64_t final_len;      // whole-message lengths for the length block
+    uint64_t final_aad_len;
 };

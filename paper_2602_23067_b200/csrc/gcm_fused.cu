@@ -210,7 +210,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         uint4 X = x;
         if (MODE != MODE_GHASH) {
             // a4 + a5: counter from the block index, then the rounds
-            const uint32_t s3 = bswap32((uint32_t)g + 2u) ^ p.rk[3];
+            const uint32_t s3 = bswap32(p.ctr_base + (uint32_t)g + 2u) ^ p.rk[3];
             const uint4 ks = aes_rounds<NR>(p, sm, lane4, p.iv_rk0[0], p.iv_rk0[1], p.iv_rk0[2], s3);
             const uint4 y = xor4(x, ks);                                   // a6
             if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
@@ -249,8 +249,14 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
     acc = cta_xor_reduce(acc, red);
     if (t == 0) {
+        if (p.chain_in != nullptr) acc = xor4(acc, gf_mul_mem(*p.chain_in, *p.chain_pow));
+        if (p.chain_out != nullptr) {       // a middle chunk of a longer message: hand the state on
+            *p.chain_out = acc;
+            *p.counter = 0;
+            return;
+        }
         // a10: length block BE64(8a) || BE64(8 len), one more multiply by H
-        const uint64_t abits = p.aad_len * 8, cbits = p.len * 8;
+        const uint64_t abits = p.final_aad_len * 8, cbits = p.final_len * 8;
         const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
                                    bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
         const uint4 S = gf_mul_mem(xor4(acc, L), __ldg(p.tab.h));

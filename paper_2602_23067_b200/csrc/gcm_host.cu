@@ -1,0 +1,193 @@
+// gcm_host.cu -- host-buffer entry points (gcm_encrypt_host / gcm_decrypt_verify_host).
+//
+// The paper's data plane stages files through pinned host memory and overlaps transfers with the
+// kernels on CUDA streams (section 3.3.2, L288-L293 section 5.2.3).  Here the
+// message is cut into chunks; chunk k travels  H2D -> fused kernel -> D2H  on stream k mod 3, so the
+// copy engines run both directions while the SMs work on another chunk.  The kernels are serialised
+// among themselves by events because each one hands the running GHASH state to the next:
+//     Y_k = Y_(k-1) . H^(n_k)  xor  Horner(chunk k)          (n_k = GHASH blocks of chunk k)
+// which is Eq. 1 regrouped; H^(n_k) comes from a small power kernel that runs
+// while the first chunk is still on the wire.
+#include <cuda_runtime.h>
+#include <string.h>
+#include <new>
+
+#include "../../include/gcm.h"
+#include "gcm_common.cuh"
+#include "gf128.cuh"
+#include "gcm_setup.cuh"
+#include "gcm_fused.cuh"
+#include "gcm_api_internal.h"
+
+#define PIPE_SLOTS 3
+#define PIPE_CHUNK_BYTES (64ull << 20)   /* multiple of 16 */
+
+struct HostPipe {
+    cudaStream_t stream[PIPE_SLOTS];
+    cudaEvent_t kernel_done[PIPE_SLOTS];
+    cudaEvent_t slot_free[PIPE_SLOTS];
+    cudaEvent_t start;
+    uint8_t *d_stage[PIPE_SLOTS];
+    uint8_t *d_aad;
+    size_t aad_cap;
+    uint4 *d_state;     // [2]: running GHASH state, ping-pong
+    uint4 *d_pows;      // [2]: H^(blocks of a full chunk), H^(blocks of the last chunk)
+};
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
+    } while (0)
+
+// out[i] = H^(e[i]) by square-and-multiply, one thread per exponent.
+__global__ void gcm_pow_kernel(const uint4 *h, uint64_t e0, uint64_t e1, uint4 *out)
+{
+    uint64_t e = threadIdx.x == 0 ? e0 : e1;
+    gf128 base = gf_from_mem(*h), r = gf_one();
+    while (e) {
+        if (e & 1) r = gf_mul(r, base);
+        base = gf_mul(base, base);
+        e >>= 1;
+    }
+    out[threadIdx.x] = gf_to_mem(r);
+}
+
+static int pipe_get(gcm_ctx *c, size_t aad_len)
+{
+    if (!c->pipe) {
+        HostPipe *hp = new (std::nothrow) HostPipe;
+        if (!hp) return GCM_ERR_NOMEM;
+        memset(hp, 0, sizeof(*hp));
+        c->pipe = hp;
+        for (int i = 0; i < PIPE_SLOTS; i++) {
+            CU(cudaStreamCreateWithFlags(&hp->stream[i], cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&hp->kernel_done[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&hp->slot_free[i], cudaEventDisableTiming));
+            CU(cudaMalloc((void **)&hp->d_stage[i], PIPE_CHUNK_BYTES));
+        }
+        CU(cudaEventCreateWithFlags(&hp->start, cudaEventDisableTiming));
+        CU(cudaMalloc((void **)&hp->d_state, 4 * sizeof(uint4)));
+        hp->d_pows = hp->d_state + 2;
+    }
+    HostPipe *hp = c->pipe;
+    if (aad_len > hp->aad_cap) {
+        if (hp->d_aad) cudaFree(hp->d_aad);
+        hp->d_aad = nullptr;
+        hp->aad_cap = 0;
+        size_t cap = (aad_len + 4095) & ~(size_t)4095;
+        CU(cudaMalloc((void **)&hp->d_aad, cap));
+        hp->aad_cap = cap;
+    }
+    return GCM_OK;
+}
+
+void gcm_host_pipe_free(gcm_ctx *c)
+{
+    HostPipe *hp = c->pipe;
+    if (!hp) return;
+    for (int i = 0; i < PIPE_SLOTS; i++) {
+        if (hp->stream[i]) cudaStreamSynchronize(hp->stream[i]);
+        if (hp->d_stage[i]) {
+            launch_wipe(hp->d_stage[i], PIPE_CHUNK_BYTES, nullptr, 0);
+            cudaDeviceSynchronize();
+            cudaFree(hp->d_stage[i]);
+        }
+        if (hp->kernel_done[i]) cudaEventDestroy(hp->kernel_done[i]);
+        if (hp->slot_free[i]) cudaEventDestroy(hp->slot_free[i]);
+        if (hp->stream[i]) cudaStreamDestroy(hp->stream[i]);
+    }
+    if (hp->start) cudaEventDestroy(hp->start);
+    if (hp->d_aad) cudaFree(hp->d_aad);
+    if (hp->d_state) cudaFree(hp->d_state);
+    delete hp;
+    c->pipe = nullptr;
+}
+
+static int run_host(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
+                    const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream)
+{
+    if (!c || !iv || !tag_io) return GCM_ERR_ARG;
+    if (len > ((1ull << 36) - 32) || aad_len >= (1ull << 32)) return GCM_ERR_LEN;
+    if ((aad_len && !h_aad) || (len && (!h_in || !h_out))) return GCM_ERR_ARG;
+    CU(cudaSetDevice(c->device));
+    int rc = pipe_get(c, aad_len);
+    if (rc != GCM_OK) return rc;
+    HostPipe *hp = c->pipe;
+    cudaStream_t us = (cudaStream_t)user_stream;
+
+    const uint64_t chunk = PIPE_CHUNK_BYTES;
+    const uint64_t n_chunks = len ? (len + chunk - 1) / chunk : 1;
+    const uint64_t last_len = len - (n_chunks - 1) * chunk;
+    // work already queued on the caller's stream happens before ours
+    CU(cudaEventRecord(hp->start, us));
+    for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamWaitEvent(hp->stream[i], hp->start, 0));
+    if (aad_len) CU(cudaMemcpyAsync(hp->d_aad, h_aad, aad_len, cudaMemcpyHostToDevice, hp->stream[0]));
+    if (n_chunks > 1) {
+        gcm_pow_kernel<<<1, 2, 0, hp->stream[PIPE_SLOTS - 1]>>>(c->d_h, chunk / 16, (last_len + 15) / 16, hp->d_pows);
+        CU(cudaGetLastError());
+        CU(cudaEventRecord(hp->kernel_done[PIPE_SLOTS - 1], hp->stream[PIPE_SLOTS - 1]));
+    }
+
+    for (uint64_t k = 0; k < n_chunks; k++) {
+        const int slot = (int)(k % PIPE_SLOTS);
+        cudaStream_t s = hp->stream[slot];
+        const uint64_t off = k * chunk;
+        const uint64_t clen = (k == n_chunks - 1) ? last_len : chunk;
+        const bool first = (k == 0), last = (k == n_chunks - 1);
+        if (clen) CU(cudaMemcpyAsync(hp->d_stage[slot], (const uint8_t *)h_in + off, clen, cudaMemcpyHostToDevice, s));
+        // kernels run in message order: chunk k needs chunk k-1's GHASH state (and the powers)
+        if (!first) CU(cudaStreamWaitEvent(s, hp->kernel_done[(k - 1) % PIPE_SLOTS], 0));
+        else if (n_chunks > 1) CU(cudaStreamWaitEvent(s, hp->kernel_done[PIPE_SLOTS - 1], 0));
+
+        GcmParams p;
+        int blocks = 0;
+        rc = gcm_build_params(c, mode, iv, first ? hp->d_aad : nullptr, first ? aad_len : 0,
+                              hp->d_stage[slot], clen, hp->d_stage[slot], &p, &blocks);
+        if (rc != GCM_OK) return rc;
+        p.ctr_base = (uint32_t)(off / 16);
+        p.final_len = len;
+        p.final_aad_len = aad_len;
+        if (!first) {
+            p.chain_in = hp->d_state + ((k - 1) & 1);
+            p.chain_pow = hp->d_pows + (last ? 1 : 0);
+        }
+        if (!last) p.chain_out = hp->d_state + (k & 1);
+        if (mode == MODE_DECRYPT) memcpy(p.tag_expect, tag_io, 16);
+        cudaError_t e = launch_fused(c->nr, mode, c->threads, blocks, p, s);
+        memset(&p, 0, sizeof(p));
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+        CU(cudaEventRecord(hp->kernel_done[slot], s));
+        if (clen) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
+        if (last) {
+            if (mode == MODE_ENCRYPT) CU(cudaMemcpyAsync(c->h_pinned, c->d_tag, 16, cudaMemcpyDeviceToHost, s));
+            else CU(cudaMemcpyAsync(c->h_pinned + 16, c->d_status, 4, cudaMemcpyDeviceToHost, s));
+        }
+    }
+    for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamSynchronize(hp->stream[i]));
+    if (mode == MODE_ENCRYPT) {
+        memcpy(tag_io, c->h_pinned, 16);
+        return GCM_OK;
+    }
+    int status;
+    memcpy(&status, c->h_pinned + 16, 4);
+    if (status != 0) {
+        memset(h_out, 0, len);       // payload suppression on the host copy
+        return GCM_ERR_AUTH;
+    }
+    return GCM_OK;
+}
+
+extern "C" int gcm_encrypt_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
+                                const void *h_pt, uint64_t len, void *h_ct, uint8_t tag[16], void *stream)
+{
+    return run_host(c, MODE_ENCRYPT, iv, h_aad, aad_len, h_pt, len, h_ct, tag, stream);
+}
+
+extern "C" int gcm_decrypt_verify_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
+                                       const void *h_ct, uint64_t len, void *h_pt, const uint8_t tag[16], void *stream)
+{
+    uint8_t t[16];
+    memcpy(t, tag, 16);
+    return run_host(c, MODE_DECRYPT, iv, h_aad, aad_len, h_ct, len, h_pt, t, stream);
+}

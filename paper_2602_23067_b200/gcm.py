@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "gcm_version", "gcm_set_device", "gcm_last_cuda_error", "gcm_last_cuda_error_string",
     "gcm_init", "gcm_destroy", "gcm_set_geometry", "gcm_get_geometry", "gcm_get_hash_subkey",
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
+    "gcm_encrypt_host", "gcm_decrypt_verify_host",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
 ]
 
@@ -77,6 +78,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_encrypt_async.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, vp, vp]
     L.gcm_decrypt_verify_async.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, vp, vp, vp]
     L.gcm_ghash_async.argtypes = [vp, vp, u64, vp, u64, vp, vp]
+    L.gcm_encrypt_host.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
+    L.gcm_decrypt_verify_host.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
     L.gcm_encrypt_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_batch_release.argtypes = []
@@ -213,6 +216,58 @@ def gcm_decrypt_verify_async(ctx: int, iv: bytes, aad, ct, pt, d_tag, d_status, 
         raise ValueError("d_tag must hold 16 bytes and d_status 4")
     _check(_L.gcm_decrypt_verify_async(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, t_ptr, s_ptr,
                                        _stream(stream)), "gcm_decrypt_verify_async")
+
+
+def _host(buf, writable: bool = False) -> Tuple[Optional[int], int, object]:
+    """(address or None, byte length, keep-alive) of a HOST buffer: numpy array, CPU torch tensor
+    (pinned or not), bytes / bytearray / memoryview."""
+    if buf is None:
+        return None, 0, None
+    if hasattr(buf, "data_ptr"):
+        if getattr(buf, "is_cuda", False):
+            raise TypeError("host buffer expected, got a CUDA tensor")
+        if not buf.is_contiguous():
+            raise ValueError("host buffer must be contiguous")
+        n = buf.numel() * buf.element_size()
+        return (buf.data_ptr() if n else None), n, buf
+    import numpy as np
+    if isinstance(buf, np.ndarray):
+        if not buf.flags["C_CONTIGUOUS"] or (writable and not buf.flags["WRITEABLE"]):
+            raise ValueError("host array must be contiguous (and writable for outputs)")
+        return (buf.ctypes.data if buf.nbytes else None), buf.nbytes, buf
+    if writable:
+        raise TypeError("writable host buffer expected (numpy array or CPU tensor)")
+    arr = np.frombuffer(bytes(buf), dtype=np.uint8)
+    return (arr.ctypes.data if arr.size else None), arr.size, arr
+
+
+def gcm_encrypt_host(ctx: int, iv: bytes, h_aad, h_pt, h_ct, stream=None) -> bytes:
+    """HOST buffers in and out (chunked H2D -> kernel -> D2H pipeline inside the library)."""
+    a_ptr, a_len, ka = _host(h_aad)
+    p_ptr, p_len, kp = _host(h_pt)
+    c_ptr, c_len, kc = _host(h_ct, writable=True)
+    if c_len != p_len:
+        raise ValueError("ct and pt sizes differ")
+    tag = ctypes.create_string_buffer(16)
+    _check(_L.gcm_encrypt_host(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)),
+           "gcm_encrypt_host")
+    del ka, kp, kc
+    return tag.raw
+
+
+def gcm_decrypt_verify_host(ctx: int, iv: bytes, h_aad, h_ct, h_pt, tag: bytes, stream=None) -> int:
+    a_ptr, a_len, ka = _host(h_aad)
+    c_ptr, c_len, kc = _host(h_ct)
+    p_ptr, p_len, kp = _host(h_pt, writable=True)
+    if c_len != p_len:
+        raise ValueError("ct and pt sizes differ")
+    tag = bytes(tag)
+    if len(tag) != 16:
+        raise ValueError("tag must be 16 bytes")
+    rc = _check(_L.gcm_decrypt_verify_host(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
+                "gcm_decrypt_verify_host", ok=(GCM_OK, GCM_ERR_AUTH))
+    del ka, kp, kc
+    return rc
 
 
 def gcm_ghash_async(ctx: int, aad, c, d_out, stream=None) -> None:
