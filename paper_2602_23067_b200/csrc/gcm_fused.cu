@@ -35,14 +35,36 @@ __device__ __forceinline__ uint32_t rotl32(uint32_t x, int n) { return __funnels
 // byte address of row (state byte `row` of w) in this lane's bank column: one PRMT
 #define TIDX(w, row) __byte_perm((w), lane4, 0x5504u | ((row) << 4))
 
-// Rounds 1..NR on a state that already had AddRoundKey(0) applied.  Little-endian column words.
-template <int NR>
-__device__ __forceinline__ uint4 aes_rounds(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
-                                            uint32_t s0, uint32_t s1, uint32_t s2, uint32_t s3)
+// Round-1 contribution of the three constant columns of a counter block (IV words ^ rk[0..2]):
+// twelve of the sixteen round-1 table reads do not depend on the counter and are done once per thread.
+struct CtrConst { uint32_t c0, c1, c2, c3; };
+
+__device__ __forceinline__ CtrConst ctr_const(const GcmParams &p, const uint8_t *sm, uint32_t lane4)
 {
     constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
+    const uint32_t s0 = p.iv_rk0[0], s1 = p.iv_rk0[1], s2 = p.iv_rk0[2];
+    CtrConst c;
+    c.c0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ p.rk[4];
+    c.c1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[5];
+    c.c2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[6];
+    c.c3 = lds32(sm, TIDX(s0, 1) + T1) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[7];
+    return c;
+}
+
+// E_K(IV || BE32(ctr)): a4 + a5.  Little-endian column words; the counter sits in column 3.
+template <int NR>
+__device__ __forceinline__ uint4 aes_ctr_block(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
+                                               const CtrConst &cc, uint32_t ctr)
+{
+    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
+    const uint32_t c3 = bswap32(ctr) ^ p.rk[3];
+    // round 1: only the four reads indexed by the counter column remain
+    uint32_t s0 = cc.c0 ^ lds32(sm, TIDX(c3, 3) + T3);
+    uint32_t s1 = cc.c1 ^ lds32(sm, TIDX(c3, 2) + T2);
+    uint32_t s2 = cc.c2 ^ lds32(sm, TIDX(c3, 1) + T1);
+    uint32_t s3 = cc.c3 ^ lds32(sm, TIDX(c3, 0) + T0);
 #pragma unroll
-    for (int r = 1; r < NR; r++) {
+    for (int r = 2; r < NR; r++) {
         uint32_t t0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[4 * r + 0];
         uint32_t t1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[4 * r + 1];
         uint32_t t2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[4 * r + 2];
@@ -172,6 +194,8 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     uint32_t sel[8];
 #pragma unroll
     for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
+    CtrConst cc = {0, 0, 0, 0};
+    if (MODE != MODE_GHASH && active) cc = ctr_const(p, sm, lane4);
 
     uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
@@ -210,8 +234,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         uint4 X = x;
         if (MODE != MODE_GHASH) {
             // a4 + a5: counter from the block index, then the rounds
-            const uint32_t s3 = bswap32(p.ctr_base + (uint32_t)g + 2u) ^ p.rk[3];
-            const uint4 ks = aes_rounds<NR>(p, sm, lane4, p.iv_rk0[0], p.iv_rk0[1], p.iv_rk0[2], s3);
+            const uint4 ks = aes_ctr_block<NR>(p, sm, lane4, cc, p.ctr_base + (uint32_t)g + 2u);
             const uint4 y = xor4(x, ks);                                   // a6
             if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
             else if (cbytes) store_bytes(p.out + 16 * g, y, cbytes);
@@ -244,6 +267,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     if (MODE != MODE_GHASH && !active) {
         fill_aes_tables<TPB>(sm, p.tab.te0);
         __syncthreads();
+        cc = ctr_const(p, sm, lane4);
     }
     uint4 acc = make_uint4(0, 0, 0, 0);
     for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
@@ -264,7 +288,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             *p.tag_out = S;
         } else {
             // a3 + a11: E_K(J0), J0 = IV || 0^31 || 1; tag; constant-time compare
-            const uint4 ek = aes_rounds<NR>(p, sm, lane4, p.iv_rk0[0], p.iv_rk0[1], p.iv_rk0[2], bswap32(1u) ^ p.rk[3]);
+            const uint4 ek = aes_ctr_block<NR>(p, sm, lane4, cc, 1u);
             const uint4 tag = xor4(S, ek);
             if (MODE == MODE_ENCRYPT) {
                 *p.tag_out = tag;
