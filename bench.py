@@ -123,11 +123,12 @@ def measured_peaks() -> dict:
 
 
 def pipe_bound_gbs(nr: int, sm_count: int, sm_mhz: float) -> dict:
-    """Shared-memory-pipe bound of the method: per 16-byte block the path needs
-    16*nr - 12 conflict-free 4-byte table reads (the 12 first-round reads of the constant IV columns
-    are hoisted) and 16 16-byte GHASH table reads = 64 bank-lanes; an SM serves 32 bank-lanes (one
-    128-byte wavefront) per cycle."""
-    lanes = 16 * nr - 12 + 64
+    """Shared-memory-pipe bound of the method.  Per 16-byte block the path needs
+    16*nr conflict-free 4-byte AES table reads minus the ones that do not depend on the low counter
+    byte (12 round-1 reads of the constant IV columns, hoisted per thread; 3 round-1 + 12 round-2
+    reads cached per lane and refreshed every 8th block: -27 + 15/8), plus 16 16-byte GHASH table
+    reads = 64 bank-lanes; an SM serves 32 bank-lanes (one 128-byte wavefront) per cycle."""
+    lanes = 16 * nr - 27 + 15.0 / 8.0 + 64
     cycles = lanes / 32.0
     return {"lanes_per_block": lanes, "cycles_per_block_per_sm": cycles,
             "gbs": sm_count * sm_mhz * 1e6 * 16.0 / cycles / 1e9}
@@ -306,7 +307,7 @@ def run_ours(args):
     pb = pipe_bound_gbs(14, sm_count, float(peaks.get("sm_max_mhz", 1965.0)))
     hbm_peak = float(peaks["hbm_gbs"])
     roofline = {
-        "bound": "alu", "pipe": "shared-memory wavefronts (LSU): %d bank-lanes per 16-byte block, 32 per SM-cycle" % pb["lanes_per_block"],
+        "bound": "alu", "pipe": "shared-memory wavefronts (LSU): %.1f bank-lanes per 16-byte block, 32 per SM-cycle" % pb["lanes_per_block"],
         "achieved": achieved, "peak": pb["gbs"], "unit": UNIT, "frac": achieved / pb["gbs"],
         "peak_source": "derived (DESIGN.md section 6): %d SMs x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s) x 16 B / %.3f cycles"
                        % (sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks["_source"], pb["cycles_per_block_per_sm"]),

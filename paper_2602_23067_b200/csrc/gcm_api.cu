@@ -56,13 +56,11 @@ static SetupParams setup_params(gcm_ctx *c, const uint8_t *key)
     memset(&sp, 0, sizeof(sp));
     if (key) memcpy(sp.key, key, c->key_bits / 8);
     sp.key_bits = c->key_bits;
-    sp.threads = c->threads;
-    sp.grid = c->grid;
     sp.te0 = c->d_te0;
     sp.rk = c->d_rk;
     sp.h = c->d_h;
     sp.hpow = c->d_hpow;
-    sp.bpow = c->d_bpow;
+    sp.hx = c->d_hx;
     sp.ktab = c->d_ktab;
     return sp;
 }
@@ -90,7 +88,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
     size_t o_te0 = take(256 * 4), o_rk = take(64 * 4), o_h = take(16);
-    size_t o_hpow = take((GCM_MAX_THREADS + 1) * 16), o_bpow = take((GCM_MAX_GRID + 1) * 16);
+    size_t o_hpow = take((GCM_STRIDE + 1) * 16), o_hx = take(HX_ENTRIES * 16);
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
     size_t o_cnt = take(4), o_tag = take(16), o_status = take(4);
     c->slab_bytes = off;
@@ -100,7 +98,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     c->d_rk = (uint32_t *)(c->d_slab + o_rk);
     c->d_h = (uint4 *)(c->d_slab + o_h);
     c->d_hpow = (uint4 *)(c->d_slab + o_hpow);
-    c->d_bpow = (uint4 *)(c->d_slab + o_bpow);
+    c->d_hx = (uint4 *)(c->d_slab + o_hx);
     c->d_ktab = (uint4 *)(c->d_slab + o_ktab);
     c->d_partials = (uint4 *)(c->d_slab + o_part);
     c->d_counter = (unsigned *)(c->d_slab + o_cnt);
@@ -151,14 +149,9 @@ extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)
     if (grid == 0) grid = c->sm_count;
     if (threads == 0) threads = GCM_MAX_THREADS;
     if (grid < 1 || grid > GCM_MAX_GRID || (threads != 256 && threads != 512)) return GCM_ERR_ARG;
-    CU(cudaSetDevice(c->device));
-    if (grid == c->grid && threads == c->threads) return GCM_OK;
+    // no table depends on the geometry: the GHASH stride power is H^32 for every launch shape
     c->grid = grid;
     c->threads = threads;
-    SetupParams sp = setup_params(c, nullptr);
-    launch_regeometry(sp, 0);
-    CU(cudaGetLastError());
-    CU(cudaDeviceSynchronize());
     return GCM_OK;
 }
 
@@ -178,9 +171,10 @@ extern "C" int gcm_get_hash_subkey(const gcm_ctx *c, uint8_t h[16])
     return GCM_OK;
 }
 
-// Argument checks and launch parameters common to encrypt / decrypt / ghash.
+// Argument checks and launch parameters common to encrypt / decrypt / ghash.  ctr_base: index of
+// the first payload block of this launch within its message (0 except in the chunked host pipeline).
 int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
-                        const void *d_in, uint64_t len, void *d_out, GcmParams *p, int *blocks)
+                     const void *d_in, uint64_t len, void *d_out, uint32_t ctr_base, GcmParams *p, int *blocks)
 {
     if (!c) return GCM_ERR_ARG;
     if (mode != MODE_GHASH && !iv) return GCM_ERR_ARG;
@@ -203,34 +197,44 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     p->aad_len = aad_len;
     p->final_len = len;
     p->final_aad_len = aad_len;
-    p->n_full = len / 16;
-    const uint64_t n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
-    const uint64_t T = (uint64_t)c->threads;
-    const uint64_t total = n_blocks + n_aad;
-    const uint64_t rows = (total + T - 1) / T;
-    if (n_aad > 0xFFFFFFFFull || rows > 0xFFFFFFFFull) return GCM_ERR_LEN;
-    p->rows = (uint32_t)rows;
-    p->pad = (uint32_t)(rows * T - total);
+    const uint64_t n_full = len / 16, n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
+    if (n_aad > 0xFFFFFFFFull) return GCM_ERR_LEN;
+    // leading zero blocks (free in GHASH) make counter == virtual index (mod 32)
+    const uint32_t pad = (2u + ctr_base - (uint32_t)n_aad) & (GCM_STRIDE - 1);
+    const uint64_t base = (uint64_t)pad + n_aad;
+    const uint64_t E = base + n_blocks;
+    if (E >= GCM_MAX_VBLOCKS) return GCM_ERR_LEN;
+    const uint64_t S = (E + GCM_STRIDE - 1) / GCM_STRIDE;
+    const uint64_t wpc = (uint64_t)c->threads / 32;              // warps per CTA
+    const uint64_t W = (uint64_t)c->grid * wpc;
+    uint64_t Q = (S + W - 1) / W;
+    if (Q < 1) Q = 1;
+    p->pad = pad;
     p->n_aad_blocks = (uint32_t)n_aad;
-    p->base = (uint64_t)p->pad + n_aad;
-    p->grid_stride = (uint32_t)c->grid;
+    p->base = base;
+    p->vblocks = E;
+    p->rows = (uint32_t)S;
+    p->rows_per_warp = (uint32_t)Q;
+    p->ctr_delta = ctr_base + 2u - (uint32_t)base;
     p->aligned = (((a | (mode == MODE_GHASH ? 0 : b)) & 15) == 0) ? 1u : 0u;
     if (p->aligned) {
-        p->fast_lo = (uint32_t)((p->base + T - 1) / T);
-        p->fast_hi = (uint32_t)((p->n_full + p->base) / T);
+        p->fast_lo = (uint32_t)((base + GCM_STRIDE - 1) / GCM_STRIDE);
+        p->fast_hi = (uint32_t)((base + n_full) / GCM_STRIDE);
         if (p->fast_hi < p->fast_lo) p->fast_hi = p->fast_lo;
     }
     p->tab.te0 = c->d_te0;
     p->tab.ktab = c->d_ktab;
     p->tab.hpow = c->d_hpow;
-    p->tab.bpow = c->d_bpow;
+    p->tab.hx = c->d_hx;
     p->tab.h = c->d_h;
     p->partials = c->d_partials;
     p->counter = c->d_counter;
     p->tag_out = c->d_tag;
     p->status = c->d_status;
-    uint64_t want = rows < 1 ? 1 : rows;
-    *blocks = (int)(want < (uint64_t)c->grid ? want : (uint64_t)c->grid);
+    const uint64_t active_warps = (S + Q - 1) / Q;
+    uint64_t want = (active_warps + wpc - 1) / wpc;
+    if (want < 1) want = 1;
+    *blocks = (int)want;
     return GCM_OK;
 }
 
@@ -240,7 +244,7 @@ extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d
     GcmParams p;
     int blocks = 0;
     if (!d_tag) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, 0, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_tag;
     CU(cudaSetDevice(c->device));
@@ -257,7 +261,7 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
     GcmParams p;
     int blocks = 0;
     if (!d_tag || !d_status) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_in = (const uint4 *)d_tag;
     p.status = (int *)d_status;
@@ -277,7 +281,7 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     GcmParams p;
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_out;
     CU(cudaSetDevice(c->device));
@@ -305,7 +309,7 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
     if (!c || !tag) return GCM_ERR_ARG;
     GcmParams p;
     int blocks = 0;
-    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, &p, &blocks);
     if (rc != GCM_OK) return rc;
     memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
     CU(cudaSetDevice(c->device));

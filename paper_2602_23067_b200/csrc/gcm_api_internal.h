@@ -10,8 +10,8 @@ struct gcm_ctx {
     int key_bits;
     int nr;            // 10 / 14
     int sm_count;
-    int grid;          // G: CTAs of the fused kernel (default: one per SM)
-    int threads;       // T: threads per CTA (512 default, 256 alternative)
+    int grid;          // CTAs of the fused kernel at most (default: one per SM)
+    int threads;       // threads per CTA (512 default, 256 alternative)
     // device state, one slab
     uint8_t  *d_slab;
     size_t    slab_bytes;
@@ -19,7 +19,7 @@ struct gcm_ctx {
     uint32_t *d_rk;
     uint4    *d_h;
     uint4    *d_hpow;
-    uint4    *d_bpow;
+    uint4    *d_hx;
     uint4    *d_ktab;
     uint4    *d_partials;
     unsigned *d_counter;
@@ -34,5 +34,5 @@ struct gcm_ctx {
 int gcm_cuda_fail(cudaError_t e);
 struct GcmParams;
 int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
-                     const void *d_in, uint64_t len, void *d_out, GcmParams *p, int *blocks);
+                     const void *d_in, uint64_t len, void *d_out, uint32_t ctr_base, GcmParams *p, int *blocks);
 void gcm_host_pipe_free(gcm_ctx *c);

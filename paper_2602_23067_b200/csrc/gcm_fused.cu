@@ -1,21 +1,27 @@
 // gcm_fused.cu -- the hot path: SURVEY.md 8(a) steps a3-a11 in ONE kernel.
 //
 //   AES-CTR keystream (a4, a5) -> XOR into the payload (a6) -> GHASH of the ciphertext while it is
-//   still in registers (a7) -> per-thread / CTA / cross-CTA combination with precomputed powers of
-//   H (a8, a9) -> AAD + length block, E_K(J0), tag, constant-time compare
-//   (a10, a11).
+//   still in registers (a7) -> per-thread / warp / CTA / cross-CTA combination with precomputed
+//   powers of H (a8, a9) -> AAD + length block, E_K(J0), tag,
+//   constant-time compare (a10, a11).
 //
 // What differs from the paper's kernels (prior art for Ampere/Ada/Hopper):
 //   * one fused pass instead of an AES-CTR kernel followed by a GHASH kernel (the ciphertext never
 //     crosses HBM twice);
-//   * the "tree" is flattened: virtual block v = row*T + t (T threads per CTA, rows dealt round-robin
-//     to the G CTAs) so every thread runs the SAME recurrence  Y <- Y.K xor X  with the one fixed
-//     multiplier K = H^(G*T), then is corrected once by H^(T-t), the CTA by (H^T)^e, and the CTA
-//     partials are XORed by the last CTA to finish.  The sum is the paper's sum of X_i . H^(N-i+1);
-//     only the association differs, and the field is exact, so the bits are identical;
+//   * the "tree" is flattened.  The virtual block sequence [pad | AAD | payload] is cut into rows of
+//     32 blocks; a warp owns a contiguous run of rows and lane l of the warp the l-th block of each.
+//     Every lane therefore runs the SAME recurrence  Y <- Y.K xor X  with the one fixed multiplier
+//     K = H^32 (independent of the launch geometry and of the message), and is corrected once by
+//     H^(1..32), the warp by H^(blocks behind the warp's run), and the partials are XORed by the
+//     last CTA to finish.  The sum is the paper's sum of X_i . H^(N-i+1); only the association
+//     differs, and the field is exact, so the bits are identical;
 //   * the multiply by the fixed K is an 8-bit Shoup table in shared memory (conflict-free by lane
 //     rotation), AES rounds are T-tables replicated per lane (conflict-free, constant-time).  On
-//     sm_100a the binding unit is the shared-memory pipe: 16*NR + 64 wavefront-lanes per block.
+//     sm_100a the binding unit is the shared-memory pipe;
+//   * counters of a lane's consecutive blocks differ by 32, so for 8 rows at a time only the low
+//     counter byte changes: of rounds 1 and 2 only 1 + 4 table reads depend on it, the other 3 + 12
+//     are cached per lane and refreshed every 8th row (in addition to the 12 round-1 reads of the
+//     constant IV columns, done once per thread).
 //
 // Counter block of payload block g is IV || BE32(g + 2): a function of g only.
 #include "gcm_common.cuh"
@@ -51,20 +57,43 @@ __device__ __forceinline__ CtrConst ctr_const(const GcmParams &p, const uint8_t 
     return c;
 }
 
-// E_K(IV || BE32(ctr)): a4 + a5.  Little-endian column words; the counter sits in column 3.
-template <int NR>
-__device__ __forceinline__ uint4 aes_ctr_block(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
-                                               const CtrConst &cc, uint32_t ctr)
+// Rounds 1-2 state that depends only on the upper 24 counter bits (see the header): the parts of the
+// four round-2 output columns that do not come from round-1 column 0.
+struct CtrCache { uint32_t u0, u1, u2, u3; };
+
+__device__ __forceinline__ CtrCache ctr_cache(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
+                                              const CtrConst &cc, uint32_t ctr)
 {
     constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
     const uint32_t c3 = bswap32(ctr) ^ p.rk[3];
-    // round 1: only the four reads indexed by the counter column remain
-    uint32_t s0 = cc.c0 ^ lds32(sm, TIDX(c3, 3) + T3);
-    uint32_t s1 = cc.c1 ^ lds32(sm, TIDX(c3, 2) + T2);
-    uint32_t s2 = cc.c2 ^ lds32(sm, TIDX(c3, 1) + T1);
-    uint32_t s3 = cc.c3 ^ lds32(sm, TIDX(c3, 0) + T0);
+    const uint32_t s1 = cc.c1 ^ lds32(sm, TIDX(c3, 2) + T2);
+    const uint32_t s2 = cc.c2 ^ lds32(sm, TIDX(c3, 1) + T1);
+    const uint32_t s3 = cc.c3 ^ lds32(sm, TIDX(c3, 0) + T0);
+    CtrCache u;
+    u.u0 = lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[8];
+    u.u1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ p.rk[9];
+    u.u2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[10];
+    u.u3 = lds32(sm, TIDX(s3, 0) + T0) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[11];
+    return u;
+}
+
+// E_K(IV || BE32(ctr)): a4 + a5.  Little-endian column words; the counter sits in column 3.  `u`
+// must have been made by ctr_cache() from a counter with the same upper 24 bits.
+template <int NR>
+__device__ __forceinline__ uint4 aes_ctr_block(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
+                                               const CtrConst &cc, const CtrCache &u, uint32_t ctr)
+{
+    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
+    // round 1: only column 0 depends on the low counter byte (state byte 15 = byte 3 of column 3)
+    const uint32_t c3 = (ctr << 24) ^ p.rk[3];
+    const uint32_t r0 = cc.c0 ^ lds32(sm, TIDX(c3, 3) + T3);
+    // round 2: one read per column is indexed by round-1 column 0
+    uint32_t s0 = u.u0 ^ lds32(sm, TIDX(r0, 0) + T0);
+    uint32_t s1 = u.u1 ^ lds32(sm, TIDX(r0, 3) + T3);
+    uint32_t s2 = u.u2 ^ lds32(sm, TIDX(r0, 2) + T2);
+    uint32_t s3 = u.u3 ^ lds32(sm, TIDX(r0, 1) + T1);
 #pragma unroll
-    for (int r = 2; r < NR; r++) {
+    for (int r = 3; r < NR; r++) {
         uint32_t t0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[4 * r + 0];
         uint32_t t1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[4 * r + 1];
         uint32_t t2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[4 * r + 2];
@@ -173,6 +202,23 @@ __device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const uint32_t *te0
     }
 }
 
+// H^d for d < 2^36 from the radix-512 digit table: four factors, two multiply levels, every lane
+// of the warp takes part (lane & 3 picks the digit) and ends up with the product.
+__device__ __forceinline__ uint4 warp_h_power(const uint4 *hx, uint64_t d, uint32_t lane)
+{
+    const uint32_t k = lane & 3;
+    const uint32_t digit = (uint32_t)(d >> (HX_RADIX_BITS * k)) & ((1u << HX_RADIX_BITS) - 1);
+    uint4 f = __ldg(hx + (k << HX_RADIX_BITS) + digit);
+#pragma unroll
+    for (int o = 1; o <= 2; o <<= 1) {
+        uint4 g;
+        g.x = __shfl_xor_sync(0xFFFFFFFFu, f.x, o); g.y = __shfl_xor_sync(0xFFFFFFFFu, f.y, o);
+        g.z = __shfl_xor_sync(0xFFFFFFFFu, f.z, o); g.w = __shfl_xor_sync(0xFFFFFFFFu, f.w, o);
+        f = gf_mul_mem(f, g);
+    }
+    return f;
+}
+
 template <int NR, int MODE, int TPB>
 __global__ void __launch_bounds__(TPB, 1)
 gcm_fused_kernel(const __grid_constant__ GcmParams p)
@@ -180,43 +226,58 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     extern __shared__ __align__(1024) uint8_t sm[];
     __shared__ bool s_last;
     const uint32_t t = threadIdx.x, lane = t & 31, lane4 = lane * 4;
-    const uint32_t G = p.grid_stride, c = blockIdx.x;
-    const bool active = c < p.rows;
+    // broadcast from lane 0: tells the compiler the warp index (and the row loop below) is warp-uniform,
+    // so the shared-memory base stays in a uniform register and folds into every LDS address
+    const uint32_t warp = __shfl_sync(0xFFFFFFFFu, t >> 5, 0);
     uint4 *red = reinterpret_cast<uint4 *>(sm + RED_OFF);
 
-    if (active) {
-        if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
+    // this warp's run of rows (a8: geometry-agnostic, the result does not depend on it)
+    const uint32_t S = p.rows, Q = p.rows_per_warp;
+    const uint64_t wg = (uint64_t)blockIdx.x * (TPB / 32) + warp;
+    const uint64_t r0_64 = wg * Q;
+    const uint32_t r0 = r0_64 < S ? (uint32_t)r0_64 : S;
+    const uint32_t r1 = (uint64_t)r0 + Q < S ? r0 + Q : S;
+    const bool has_rows = r0 < r1;
+
+    if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
+    {
         uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
         for (uint32_t j = t; j < KTAB_BYTES / 16; j += TPB) kt[j] = __ldg(p.tab.ktab + j);
     }
+    // position weight of the warp's run, H^(blocks behind it): computed while the tables arrive
+    uint4 wpow = make_uint4(0, 0, 0, 0);
+    const bool tail_warp = has_rows && r1 == S;          // owns the last (possibly ragged) row
+    if (has_rows && !tail_warp) wpow = warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane);
     __syncthreads();
 
     uint32_t sel[8];
 #pragma unroll
     for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
     CtrConst cc = {0, 0, 0, 0};
-    if (MODE != MODE_GHASH && active) cc = ctr_const(p, sm, lane4);
+    CtrCache cu = {0, 0, 0, 0};
+    if (MODE != MODE_GHASH) cc = ctr_const(p, sm, lane4);
 
     uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
     bool have_pre = false;
-    const uint64_t row_bytes = (uint64_t)G * TPB * 16;
 
-    for (uint32_t row = c; row < p.rows; row += G) {
-        const uint64_t v = (uint64_t)row * TPB + t;     // virtual block index
+    for (uint32_t row = r0; row < r1; row++) {
+        const uint64_t v = 32ull * row + lane;          // virtual block index
         const bool fast = row >= p.fast_lo && row < p.fast_hi;
         uint4 x = make_uint4(0, 0, 0, 0);
-        uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD)
+        uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD / beyond the end)
         uint64_t g = 0;                                 // payload block index
+        bool valid = true;
         if (fast) {
             g = v - p.base;
             x = have_pre ? pre : ld16_stream(p.in + 16 * g);
             cbytes = 16;
-            have_pre = row + G < p.fast_hi;
-            if (have_pre) pre = ld16_stream(p.in + 16 * g + row_bytes);
+            have_pre = row + 1 < r1 && row + 1 < p.fast_hi;
+            if (have_pre) pre = ld16_stream(p.in + 16 * g + 512);
         } else {
             have_pre = false;
-            if (v >= p.pad) {
+            valid = v < p.vblocks;
+            if (valid && v >= p.pad) {
                 const uint64_t u = v - p.pad;
                 if (u < p.n_aad_blocks) {
                     const uint64_t rem = p.aad_len - 16 * u;
@@ -233,30 +294,47 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         const uint4 ym = ghash_mul_k(sm, sel, Y);
         uint4 X = x;
         if (MODE != MODE_GHASH) {
-            // a4 + a5: counter from the block index, then the rounds
-            const uint4 ks = aes_ctr_block<NR>(p, sm, lane4, cc, p.ctr_base + (uint32_t)g + 2u);
+            // a4: counter from the virtual index alone; the upper 24 bits are warp-uniform and change
+            // every 8th row, when rounds 1-2 are re-cached
+            const uint32_t ctr = (uint32_t)v + p.ctr_delta;
+            if (row == r0 || (ctr & 0xE0u) == 0) cu = ctr_cache(p, sm, lane4, cc, ctr);
+            const uint4 ks = aes_ctr_block<NR>(p, sm, lane4, cc, cu, ctr);     // a5
             const uint4 y = xor4(x, ks);                                   // a6
             if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
             else if (cbytes) store_bytes(p.out + 16 * g, y, cbytes);
             if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
         }
-        Y = xor4(ym, X);
+        if (fast || valid) Y = xor4(ym, X);
     }
 
-    // a8: per-thread correction by H^(T - t), XOR over the CTA, CTA correction by (H^T)^e
+    // a8: lane correction H^(blocks from the lane's last block to the end of the warp's run), XOR over
+    // the warp, warp correction H^(blocks behind the run), XOR over the CTA.  In the ragged last row
+    // only lanes < rem folded a block; rotating the lane order by rem keeps the exponents in 1..32.
     uint4 part = make_uint4(0, 0, 0, 0);
-    if (active) {
-        const uint4 yc = gf_mul_mem(Y, __ldg(p.tab.hpow + (TPB - t)));
-        part = cta_xor_reduce(yc, red);
-        if (t == 0) {
-            const uint32_t last = c + G * ((p.rows - 1 - c) / G);
-            const uint32_t e = p.rows - 1 - last;
-            if (e) part = gf_mul_mem(part, __ldg(p.tab.bpow + e));
+    if (has_rows) {
+        const uint32_t rem = tail_warp ? (uint32_t)(p.vblocks - 32ull * (S - 1)) : 32u;   // 1..32
+        const uint32_t e = ((rem - lane - 1) & 31) + 1;
+        part = gf_mul_mem(Y, __ldg(p.tab.hpow + e));
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        part.x ^= __shfl_xor_sync(0xFFFFFFFFu, part.x, o); part.y ^= __shfl_xor_sync(0xFFFFFFFFu, part.y, o);
+        part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
+    }
+    if (has_rows && !tail_warp) part = gf_mul_mem(part, wpow);
+    if (lane == 0) red[warp] = part;
+    __syncthreads();
+    if (warp == 0) {
+        part = lane < TPB / 32 ? red[lane] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            part.x ^= __shfl_xor_sync(0xFFFFFFFFu, part.x, o); part.y ^= __shfl_xor_sync(0xFFFFFFFFu, part.y, o);
+            part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
         }
     }
     // a9: last-CTA-done combination of the partials
     if (t == 0) {
-        p.partials[c] = part;
+        p.partials[blockIdx.x] = part;
         __threadfence();
         const unsigned ticket = atomicAdd(p.counter, 1u);
         s_last = (ticket == gridDim.x - 1);
@@ -264,11 +342,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    if (MODE != MODE_GHASH && !active) {
-        fill_aes_tables<TPB>(sm, p.tab.te0);
-        __syncthreads();
-        cc = ctr_const(p, sm, lane4);
-    }
     uint4 acc = make_uint4(0, 0, 0, 0);
     for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
     acc = cta_xor_reduce(acc, red);
@@ -283,13 +356,14 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         const uint64_t abits = p.final_aad_len * 8, cbits = p.final_len * 8;
         const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
                                    bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
-        const uint4 S = gf_mul_mem(xor4(acc, L), __ldg(p.tab.h));
+        const uint4 Sg = gf_mul_mem(xor4(acc, L), __ldg(p.tab.h));
         if (MODE == MODE_GHASH) {
-            *p.tag_out = S;
+            *p.tag_out = Sg;
         } else {
             // a3 + a11: E_K(J0), J0 = IV || 0^31 || 1; tag; constant-time compare
-            const uint4 ek = aes_ctr_block<NR>(p, sm, lane4, cc, 1u);
-            const uint4 tag = xor4(S, ek);
+            cu = ctr_cache(p, sm, lane4, cc, 1u);
+            const uint4 ek = aes_ctr_block<NR>(p, sm, lane4, cc, cu, 1u);
+            const uint4 tag = xor4(Sg, ek);
             if (MODE == MODE_ENCRYPT) {
                 *p.tag_out = tag;
             } else {

@@ -143,9 +143,8 @@ static int run_host(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, 
         GcmParams p;
         int blocks = 0;
         rc = gcm_build_params(c, mode, iv, first ? hp->d_aad : nullptr, first ? aad_len : 0,
-                              hp->d_stage[slot], clen, hp->d_stage[slot], &p, &blocks);
+                              hp->d_stage[slot], clen, hp->d_stage[slot], (uint32_t)(off / 16), &p, &blocks);
         if (rc != GCM_OK) return rc;
-        p.ctr_base = (uint32_t)(off / 16);
         p.final_len = len;
         p.final_aad_len = aad_len;
         if (!first) {

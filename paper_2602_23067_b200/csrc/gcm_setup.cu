@@ -1,6 +1,6 @@
 // gcm_setup.cu -- steps a1 + a2 of SURVEY.md 8(a): key schedule, H = E_K(0^128), the powers of H
 // and the multiplier table of the fixed stride power (the table of
-// powers of the hash key is generated on the GPU).  One CTA, runs once per key / geometry.
+// powers of the hash key is generated on the GPU).  One CTA, runs once per key.
 // Not hot.  Everything is computed from definitions; no typed-in tables.
 #include "gcm_common.cuh"
 #include "gf128.cuh"
@@ -129,21 +129,27 @@ gcm_setup_kernel(SetupParams p)
         p.h[0] = h;
     }
     __syncthreads();
-    gcm_build_power_tables(p.h[0], p.threads, p.grid, p.hpow, p.bpow, p.ktab, s_v);
+    gcm_build_power_tables(p.h[0], p.hpow, p.hx, p.ktab, s_v);
 }
 
-// Everything that depends on H and the geometry: hpow[i] = H^i (i <= threads), bpow[j] = B^j with
-// B = H^threads (j <= grid), K = B^grid = H^(threads*grid), and the Shoup table of K.
-__device__ void gcm_build_power_tables(uint4 h, int threads, int grid, uint4 *hpow, uint4 *bpow, uint4 *ktab, uint4 *s_v)
+// Everything that depends on H only: hpow[i] = H^i (i <= 32), the radix-512 position-weight powers
+// hx[k*512 + j] = H^(j * 512^k), K = H^32 and the Shoup table of K.
+__device__ void gcm_build_power_tables(uint4 h, uint4 *hpow, uint4 *hx, uint4 *ktab, uint4 *s_v)
 {
     const int t = threadIdx.x;
-    power_table(hpow, h, threads);
-    power_table(bpow, hpow[threads], grid);
+    power_table(hpow, h, GCM_STRIDE);
+    uint4 base = h;
+    for (int k = 0; k < HX_DIGITS; k++) {
+        uint4 *tab = hx + (k << HX_RADIX_BITS);
+        power_table(tab, base, (1 << HX_RADIX_BITS) - 1);
+        base = gf_mul_mem(tab[(1 << HX_RADIX_BITS) - 1], base);     // base^(512): next digit's base
+        __syncthreads();
+    }
     // V_i = K . x^i, i = 0..127 ("mem" format): the images of the basis vectors
     if (t < 128) {
         gf128 e = gf_zero();
         e.w[t >> 5] = 1u << (31 - (t & 31));
-        s_v[t] = gf_to_mem(gf_mul(e, gf_from_mem(bpow[grid])));
+        s_v[t] = gf_to_mem(gf_mul(e, gf_from_mem(hpow[GCM_STRIDE])));
     }
     __syncthreads();
     // entry (P, v) = XOR over the set bits b of v of V[8P + 7 - b]  (bit 7 of a byte is the lowest power)
@@ -154,14 +160,6 @@ __device__ void gcm_build_power_tables(uint4 h, int threads, int grid, uint4 *hp
             if ((v >> b) & 1) acc = xor4(acc, s_v[8 * P + 7 - b]);
         ktab[v * 16 + (P >> 3) * 8 + (P & 7)] = acc;
     }
-}
-
-// Rebuild only the geometry-dependent tables (gcm_set_geometry).
-__global__ void __launch_bounds__(512, 1)
-gcm_regeometry_kernel(SetupParams p)
-{
-    __shared__ uint4 s_v[128];
-    gcm_build_power_tables(p.h[0], p.threads, p.grid, p.hpow, p.bpow, p.ktab, s_v);
 }
 
 // Overwrite a buffer with zeros: key material on destroy, and the plaintext on authentication
@@ -183,7 +181,6 @@ __global__ void gcm_wipe_kernel(uint8_t *dst, uint64_t len, const int *status)
 }
 
 void launch_setup(const SetupParams &p, cudaStream_t s) { gcm_setup_kernel<<<1, 512, 0, s>>>(p); }
-void launch_regeometry(const SetupParams &p, cudaStream_t s) { gcm_regeometry_kernel<<<1, 512, 0, s>>>(p); }
 void launch_wipe(uint8_t *dst, uint64_t len, const int *status, cudaStream_t s)
 {
     if (len == 0) return;
