@@ -186,10 +186,7 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
 
     memset(p, 0, sizeof(*p));
     memcpy(p->rk, c->h_rk, sizeof(p->rk));
-    if (iv) {
-        memcpy(p->iv, iv, 12);
-        for (int i = 0; i < 3; i++) p->iv_rk0[i] = p->iv[i] ^ p->rk[i];
-    }
+    if (iv) memcpy(p->iv, iv, 12);
     p->in = (const uint8_t *)d_in;
     p->out = (uint8_t *)d_out;
     p->aad = (const uint8_t *)d_aad;

@@ -1,80 +1,486 @@
-// gcm_batch.cu -- batched many-message entry points (include/gcm.h).
+// gcm_batch.cu -- batched many-message entry points (include/gcm.h; SURVEY.md 3.5, 8(a) with the
+// per-message rows a1-a3 done 10,000 times for config C4).
+//
+// Small messages (< BATCH_LARGE_BYTES): ONE persistent kernel, one WARP per message.  A warp takes
+// the next message from a ticket counter and runs the whole path on it with no CTA-wide step:
+//   a1  key expansion from the lane-replicated round tables (all lanes redundantly: same cost as one)
+//   a2  H = E_K(0), the ladder H^(2^k), k = 0..5, by squaring ("table of powers of
+//       the hash key H^(2^0), H^(2^1), ..."), and a 4-bit Shoup table of K = H^32 in the warp's own
+//       8 KB of shared memory (512 entries: cheap enough to build per message, unlike the 8-bit one)
+//   a3  E_K(J0) next to H (lane 0 encrypts 0^128, lane 1 encrypts J0)
+//   a4-a7  rows of 32 blocks exactly as in the fused kernel: cached counter rounds, T-table rounds,
+//       XOR, Y <- Y.K xor X with the ciphertext still in registers
+//   a8  the paper's binary tree (Fig. 3b) across the 32 lanes: at level k the left
+//       partial is multiplied by H^(2^k) and XORed into the right one
+//   a10-a11  length block, tag, constant-time compare, zero-fill of the output on mismatch.
+// Keys never touch global memory except inside the descriptor array, which is wiped after the call.
 //
 // Large messages (FITS-sized HDUs, config C3) go through the fused single-message kernel with a
-// per-key context that is cached across calls, one launch per message on the caller's stream.
+// per-key context that is cached across calls, one asynchronous launch per message on the caller's
+// stream; tags and verdicts of both paths come back in one copy.
 #include <cuda_runtime.h>
 #include <string.h>
+#include <algorithm>
 #include <map>
+#include <mutex>
+#include <new>
 #include <string>
 #include <vector>
-#include <mutex>
 
 #include "../../include/gcm.h"
 #include "gcm_common.cuh"
+#include "gcm_device.cuh"
+#include "gcm_setup.cuh"
 #include "gcm_api_internal.h"
 
-namespace {
-struct KeyCache {
-    std::mutex mu;
-    std::map<std::string, gcm_ctx *> by_key;   // key bytes (+ device) -> context
-    std::vector<std::string> order;            // insertion order, for eviction
-    static constexpr size_t kMax = 64;
-};
-KeyCache g_cache;
+#define BATCH_WARPS        12
+#define BATCH_THREADS      (32 * BATCH_WARPS)
+#define BATCH_TAB_OFF      AES_TAB_BYTES                 /* per-warp 4-bit tables: 8 KB each */
+#define BATCH_TAB_BYTES    8192
+#define BATCH_HP_OFF       (BATCH_TAB_OFF + BATCH_WARPS * BATCH_TAB_BYTES)   /* per warp: H^(2^k), k = 0..4 */
+#define BATCH_HP_BYTES     128
+#define BATCH_SMEM_BYTES   (BATCH_HP_OFF + BATCH_WARPS * BATCH_HP_BYTES)
+#define BATCH_LARGE_BYTES  (256ull << 10)                /* at and above: fused kernel per message */
 
-void evict_all_locked()
+struct BatchDesc {            // one per message, device; 112 bytes so that tag stays 16-byte aligned
+    uint32_t key[8];
+    uint32_t tag[4];          // decrypt: expected tag
+    uint32_t iv[3];
+    uint32_t pad32;
+    const uint8_t *aad;
+    const uint8_t *in;
+    uint8_t *out;
+    uint64_t aad_len;
+    uint64_t len;
+    uint64_t pad64;
+};
+static_assert(sizeof(BatchDesc) == 112, "BatchDesc layout");
+struct BatchResult {          // one per message, device
+    uint32_t tag[4];
+    int status;
+    int pad[3];
+};
+
+// ---- device ---------------------------------------------------------------------------------------
+
+// y . K through the warp's 4-bit table.  Entry (P, v), P = nibble position 0..31 (nibble P holds the
+// coefficients of x^(4P) .. x^(4P+3), highest bit first), is stored at v*512 + (P>>3)*128 + (P&7)*16.
+// In step r lane q looks at nibble 8*(r>>3) + ((q + r) & 7): the eight lanes of an LDS.128 phase hit
+// eight different 16-byte columns whatever the nibble values are (conflict-free, constant-time).
+// rot[k], col[k] (k = r & 7): rotation that brings that nibble to bits 9..12, and the column offset.
+__device__ __forceinline__ uint4 ghash_mul4(const uint8_t *tab, const uint32_t (&rot)[8], const uint32_t (&col)[8], uint4 y)
 {
-    for (auto &kv : g_cache.by_key) gcm_destroy(kv.second);
-    g_cache.by_key.clear();
-    for (auto &s : g_cache.order) { volatile char *v = &s[0]; for (size_t i = 0; i < s.size(); i++) v[i] = 0; }
-    g_cache.order.clear();
+    const uint32_t w[4] = {y.x, y.y, y.z, y.w};
+    uint4 acc = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int r = 0; r < 32; r++) {
+        const uint32_t x = w[r >> 3];
+        const uint32_t off = (__funnelshift_r(x, x, rot[r & 7]) & 0x1E00u) | col[r & 7];
+        acc = xor4(acc, lds128(tab, off + 128 * (r >> 3)));
+    }
+    return acc;
 }
 
-int ctx_for_key(const uint8_t *key, int key_bits, gcm_ctx **out)
+__device__ __forceinline__ uint4 shfl4(uint4 v, uint32_t src)
 {
-    if (!key || (key_bits != 128 && key_bits != 256)) return GCM_ERR_ARG;
+    return make_uint4(__shfl_sync(0xFFFFFFFFu, v.x, src), __shfl_sync(0xFFFFFFFFu, v.y, src),
+                      __shfl_sync(0xFFFFFFFFu, v.z, src), __shfl_sync(0xFFFFFFFFu, v.w, src));
+}
+
+template <int NR, int MODE>
+__device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *res, const uint8_t *sm,
+                                              uint8_t *tab, uint4 *hp, uint32_t lane)
+{
+    const uint32_t lane4 = lane * 4;
+    // a1: key expansion (registers; the same work in every lane)
+    uint32_t rk[4 * (NR + 1)];
+    aes_key_expand<NR>(sm, lane4, d.key, rk);
+    // a2 + a3: lane 0 encrypts 0^128, lane 1 encrypts J0 = IV || 0^31 || 1
+    uint4 blk = make_uint4(0, 0, 0, 0);
+    if (lane == 1) blk = make_uint4(d.iv[0], d.iv[1], d.iv[2], 0x01000000u);
+    blk = aes_encrypt_block<NR>(rk, sm, lane4, blk);
+    const uint4 h = shfl4(blk, 0), ekj0 = shfl4(blk, 1);
+    // ladder H^(2^k): k = 0..4 kept for the tree, k = 5 is the stride power K
+    gf128 hk = gf_from_mem(h);
+#pragma unroll 1
+    for (int k = 0; k < 5; k++) {
+        if (lane == 0) hp[k] = gf_to_mem(hk);
+        hk = gf_sqr(hk);
+    }
+    // 4-bit table of K: lane P owns nibble position P
+    {
+        gf128 e = gf_zero();
+        e.w[lane >> 3] = 1u << (31 - 4 * (lane & 7));            // x^(4P)
+        gf128 v0 = gf_mul(e, hk), v1 = gf_mulx(v0), v2 = gf_mulx(v1), v3 = gf_mulx(v2);
+        uint4 *row = reinterpret_cast<uint4 *>(tab + (lane >> 3) * 128 + (lane & 7) * 16);
+#pragma unroll
+        for (int v = 0; v < 16; v++) {
+            gf128 a = gf_zero();
+            if (v & 8) a = gf_xor(a, v0);
+            if (v & 4) a = gf_xor(a, v1);
+            if (v & 2) a = gf_xor(a, v2);
+            if (v & 1) a = gf_xor(a, v3);
+            row[v * 32] = gf_to_mem(a);                          // v * 512 bytes
+        }
+    }
+    __syncwarp();
+
+    uint32_t rot[8], col[8];
+#pragma unroll
+    for (int k = 0; k < 8; k++) {
+        const uint32_t n = (lane + k) & 7;
+        const uint32_t sh = 8 * (n >> 1) + ((n & 1) ? 0 : 4);    // bit position of the nibble in its word
+        rot[k] = (sh - 9) & 31;
+        col[k] = n * 16;
+    }
+
+    // the virtual block sequence [pad | AAD | payload] of the fused kernel, all rows in this warp
+    const uint64_t len = d.len, aad_len = d.aad_len;
+    const uint64_t n_full = len / 16, n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
+    const uint32_t pad = (2u - (uint32_t)n_aad) & 31;
+    const uint64_t base = pad + n_aad, E = base + n_blocks;
+    const uint32_t S = (uint32_t)((E + 31) / 32);
+    const uint32_t ctr_delta = 2u - (uint32_t)base;
+    const bool aligned = ((((uintptr_t)d.in) | ((uintptr_t)d.out)) & 15) == 0;
+    uint32_t fast_lo = 0, fast_hi = 0;
+    if (aligned) {
+        fast_lo = (uint32_t)((base + 31) / 32);
+        fast_hi = (uint32_t)((base + n_full) / 32);
+        if (fast_hi < fast_lo) fast_hi = fast_lo;
+    }
+
+    const CtrConst cc = ctr_const(rk, d.iv[0], d.iv[1], d.iv[2], sm, lane4);
+    CtrCache cu = {0, 0, 0, 0};
+    uint4 Y = make_uint4(0, 0, 0, 0), pre = make_uint4(0, 0, 0, 0);
+    bool have_pre = false;
+#pragma unroll 1
+    for (uint32_t row = 0; row < S; row++) {
+        const uint64_t v = 32ull * row + lane;
+        const bool fast = row >= fast_lo && row < fast_hi;
+        uint4 x = make_uint4(0, 0, 0, 0);
+        uint32_t cbytes = 0;
+        uint64_t g = 0;
+        bool valid = true;
+        if (fast) {
+            g = v - base;
+            x = have_pre ? pre : ld16_stream(d.in + 16 * g);
+            cbytes = 16;
+            have_pre = row + 1 < fast_hi;
+            if (have_pre) pre = ld16_stream(d.in + 16 * g + 512);
+        } else {
+            have_pre = false;
+            valid = v < E;
+            if (valid && v >= pad) {
+                const uint64_t u = v - pad;
+                if (u < n_aad) {
+                    const uint64_t rem = aad_len - 16 * u;
+                    x = load_bytes(d.aad + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
+                } else {
+                    g = u - n_aad;
+                    const uint64_t rem = len - 16 * g;
+                    cbytes = rem < 16 ? (uint32_t)rem : 16u;
+                    x = (cbytes == 16 && aligned) ? ld16_stream(d.in + 16 * g) : load_bytes(d.in + 16 * g, cbytes);
+                }
+            }
+        }
+        const uint4 ym = ghash_mul4(tab, rot, col, Y);           // a7
+        const uint32_t ctr = (uint32_t)v + ctr_delta;            // a4
+        if (row == 0 || (ctr & 0xE0u) == 0) cu = ctr_cache(rk, sm, lane4, cc, ctr);
+        const uint4 ks = aes_ctr_block<NR>(rk, sm, lane4, cc, cu, ctr);   // a5
+        const uint4 y = xor4(x, ks);                             // a6
+        if (cbytes == 16 && (fast || aligned)) st16_stream(d.out + 16 * g, y);
+        else if (cbytes) store_bytes(d.out + 16 * g, y, cbytes);
+        uint4 X = x;
+        if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
+        if (fast || valid) Y = xor4(ym, X);
+    }
+
+    // a8: the tree over the lanes, in the order of their last blocks (rotate by the ragged remainder):
+    // index i = (lane - rem) & 31 holds the partial whose last block is 31 - i blocks before the end.
+    const uint32_t rem = (uint32_t)(E - 32ull * (S ? S - 1 : 0)) & 31;      // E mod 32 (0: full last row)
+    const uint32_t i = (lane - rem) & 31;
+    uint4 Z = Y;
+#pragma unroll 1
+    for (int k = 0; k < 5; k++) {
+        const uint32_t src = ((i - (1u << k)) + rem) & 31;       // lane holding index i - 2^k
+        const uint4 left = shfl4(Z, src);
+        const uint4 prod = gf_mul_mem(left, hp[k]);
+        if ((i & ((2u << k) - 1)) == (2u << k) - 1) Z = xor4(Z, prod);
+    }
+    // index 31 (lane (31 + rem) & 31) now holds sum X_v . H^(E - 1 - v); a10: one H for the chain, then
+    // the length block and the last H
+    const uint64_t abits = aad_len * 8, cbits = len * 8;
+    const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
+                               bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
+    const uint4 acc = gf_mul_mem(Z, h);
+    const uint4 Sg = gf_mul_mem(xor4(acc, L), h);
+    const uint4 tag = shfl4(xor4(Sg, ekj0), (31 + rem) & 31);    // a11
+    if (MODE == MODE_ENCRYPT) {
+        if (lane == 0) {
+            res->tag[0] = tag.x; res->tag[1] = tag.y; res->tag[2] = tag.z; res->tag[3] = tag.w;
+            res->status = 0;
+        }
+    } else {
+        const uint32_t diff = (tag.x ^ d.tag[0]) | (tag.y ^ d.tag[1]) | (tag.z ^ d.tag[2]) | (tag.w ^ d.tag[3]);
+        if (lane == 0) res->status = diff != 0 ? 1 : 0;
+        if (diff != 0) {                                        // payload suppression
+            __syncwarp();
+            uint64_t head = (16 - ((uintptr_t)d.out & 15)) & 15;
+            if (head > len) head = len;
+            const uint64_t mid = (len - head) / 16;
+            for (uint64_t k = lane; k < head; k += 32) d.out[k] = 0;
+            uint4 *o4 = reinterpret_cast<uint4 *>(d.out + head);
+            for (uint64_t k = lane; k < mid; k += 32) o4[k] = make_uint4(0, 0, 0, 0);
+            for (uint64_t k = head + mid * 16 + lane; k < len; k += 32) d.out[k] = 0;
+        }
+    }
+}
+
+// order[j]: message index of the j-th ticket (longest first); next: ticket counter.
+template <int NR, int MODE>
+__global__ void __launch_bounds__(BATCH_THREADS, 1)
+gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *order, uint32_t n,
+                 unsigned *next, const uint32_t *te0)
+{
+    extern __shared__ __align__(1024) uint8_t sm[];
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t warp = __shfl_sync(0xFFFFFFFFu, threadIdx.x >> 5, 0);
+    fill_aes_tables<BATCH_THREADS>(sm, te0);
+    __syncthreads();
+    uint8_t *tab = sm + BATCH_TAB_OFF + warp * BATCH_TAB_BYTES;
+    uint4 *hp = reinterpret_cast<uint4 *>(sm + BATCH_HP_OFF + warp * BATCH_HP_BYTES);
+    for (;;) {
+        unsigned j = 0;
+        if (lane == 0) j = atomicAdd(next, 1u);
+        j = __shfl_sync(0xFFFFFFFFu, j, 0);
+        if (j >= n) break;
+        const uint32_t m = __ldg(order + j);
+        BatchDesc d = descs[m];
+        batch_message<NR, MODE>(d, results + m, sm, tab, hp, lane);
+        __syncwarp();
+    }
+}
+
+template <int NR, int MODE>
+static cudaError_t launch_batch(int blocks, const BatchDesc *descs, BatchResult *results, const uint32_t *order,
+                                uint32_t n, unsigned *next, const uint32_t *te0, cudaStream_t s)
+{
+    auto kern = gcm_batch_kernel<NR, MODE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, BATCH_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    kern<<<blocks, BATCH_THREADS, BATCH_SMEM_BYTES, s>>>(descs, results, order, n, next, te0);
+    return cudaGetLastError();
+}
+
+// ---- host -----------------------------------------------------------------------------------------
+namespace {
+
+struct BatchState {
+    std::mutex mu;
+    // fused-path contexts, by key bytes + device
+    std::map<std::string, gcm_ctx *> by_key;
+    static constexpr size_t kMaxKeys = 64;
+    // staging of the small-message path (one device at a time; re-made when the device changes)
+    int device = -1;
+    int sm_count = 0;
+    uint32_t cap = 0;
+    BatchDesc *h_desc = nullptr, *d_desc = nullptr;
+    BatchResult *h_res = nullptr, *d_res = nullptr;
+    uint32_t *h_order = nullptr, *d_order = nullptr;
+    unsigned *d_next = nullptr;      // [2]
+    uint32_t *d_te0 = nullptr;
+};
+BatchState g;
+
+void secure_zero(void *p, size_t n)
+{
+    volatile uint8_t *v = (volatile uint8_t *)p;
+    while (n--) *v++ = 0;
+}
+
+void free_staging_locked()
+{
+    if (g.device < 0) return;
+    cudaSetDevice(g.device);
+    if (g.d_desc) { launch_wipe((uint8_t *)g.d_desc, (uint64_t)g.cap * sizeof(BatchDesc), nullptr, 0); cudaDeviceSynchronize(); cudaFree(g.d_desc); }
+    if (g.h_desc) { secure_zero(g.h_desc, (size_t)g.cap * sizeof(BatchDesc)); cudaFreeHost(g.h_desc); }
+    if (g.d_res) cudaFree(g.d_res);
+    if (g.h_res) cudaFreeHost(g.h_res);
+    if (g.d_order) cudaFree(g.d_order);
+    if (g.h_order) cudaFreeHost(g.h_order);
+    if (g.d_next) cudaFree(g.d_next);
+    if (g.d_te0) cudaFree(g.d_te0);
+    g.d_desc = g.h_desc = nullptr; g.d_res = g.h_res = nullptr; g.d_order = g.h_order = nullptr;
+    g.d_next = nullptr; g.d_te0 = nullptr; g.cap = 0; g.device = -1;
+    cudaGetLastError();
+}
+
+void evict_keys_locked()
+{
+    for (auto &kv : g.by_key) gcm_destroy(kv.second);
+    // std::string keeps the key bytes: overwrite before the nodes are freed
+    for (auto &kv : g.by_key) secure_zero(const_cast<char *>(kv.first.data()), kv.first.size());
+    g.by_key.clear();
+}
+
+int ensure_staging_locked(uint32_t n)
+{
     int dev = 0;
-    cudaGetDevice(&dev);
-    std::string id((const char *)key, key_bits / 8);
-    id.push_back((char)dev);
-    auto it = g_cache.by_key.find(id);
-    if (it != g_cache.by_key.end()) { *out = it->second; return GCM_OK; }
-    if (g_cache.by_key.size() >= KeyCache::kMax) evict_all_locked();
-    gcm_ctx *c = nullptr;
-    int rc = gcm_init(&c, key, key_bits);
-    if (rc != GCM_OK) return rc;
-    g_cache.by_key[id] = c;
-    g_cache.order.push_back(id);
-    *out = c;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    if (g.device != dev || g.cap < n) {
+        free_staging_locked();
+        cudaDeviceProp prop;
+        if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return gcm_cuda_fail(e);
+        if ((size_t)prop.sharedMemPerBlockOptin < (size_t)BATCH_SMEM_BYTES) return GCM_ERR_CUDA;
+        g.device = dev;
+        g.sm_count = prop.multiProcessorCount;
+        uint32_t cap = 1024;
+        while (cap < n) cap *= 2;
+        do {
+            if ((e = cudaHostAlloc((void **)&g.h_desc, (size_t)cap * sizeof(BatchDesc), cudaHostAllocDefault)) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_desc, (size_t)cap * sizeof(BatchDesc))) != cudaSuccess) break;
+            if ((e = cudaHostAlloc((void **)&g.h_res, (size_t)cap * sizeof(BatchResult), cudaHostAllocDefault)) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_res, (size_t)cap * sizeof(BatchResult))) != cudaSuccess) break;
+            if ((e = cudaHostAlloc((void **)&g.h_order, (size_t)cap * sizeof(uint32_t), cudaHostAllocDefault)) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_order, (size_t)cap * sizeof(uint32_t))) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_next, 2 * sizeof(unsigned))) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_te0, 256 * sizeof(uint32_t))) != cudaSuccess) break;
+            launch_te0(g.d_te0, 0);
+            if ((e = cudaGetLastError()) != cudaSuccess) break;
+            if ((e = cudaDeviceSynchronize()) != cudaSuccess) break;
+        } while (0);
+        if (e != cudaSuccess) {
+            int rc = gcm_cuda_fail(e);
+            g.cap = cap;
+            free_staging_locked();
+            return rc;
+        }
+        g.cap = cap;
+    }
     return GCM_OK;
 }
+
+int ctx_for_key_locked(const uint8_t *key, int key_bits, cudaStream_t s, gcm_ctx **out)
+{
+    std::string id((const char *)key, key_bits / 8);
+    id.push_back((char)g.device);
+    auto it = g.by_key.find(id);
+    if (it != g.by_key.end()) { *out = it->second; secure_zero(&id[0], id.size()); return GCM_OK; }
+    if (g.by_key.size() >= BatchState::kMaxKeys) {
+        cudaStreamSynchronize(s);          // queued launches may still use the contexts
+        evict_keys_locked();
+    }
+    gcm_ctx *c = nullptr;
+    int rc = gcm_init(&c, key, key_bits);
+    if (rc == GCM_OK) { g.by_key[id] = c; *out = c; }
+    secure_zero(&id[0], id.size());
+    return rc;
+}
+
+int check_msg(const gcm_msg &m)
+{
+    if (!m.key || (m.key_bits != 128 && m.key_bits != 256)) return GCM_ERR_ARG;
+    if (m.len > ((1ull << 36) - 32) || m.aad_len >= (1ull << 61)) return GCM_ERR_LEN;
+    if ((m.aad_len && !m.d_aad) || (m.len && (!m.d_in || !m.d_out))) return GCM_ERR_ARG;
+    const uintptr_t a = (uintptr_t)m.d_in, b = (uintptr_t)m.d_out;
+    if (m.len && a != b && a < b + m.len && b < a + m.len) return GCM_ERR_ARG;
+    return GCM_OK;
+}
+
+#define CUB(call)                                                                                  \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
+    } while (0)
+
+int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
+{
+    if (n && !msgs) return GCM_ERR_ARG;
+    if (n == 0) return GCM_OK;
+    std::lock_guard<std::mutex> lock(g.mu);
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_staging_locked(n);
+    if (rc != GCM_OK) return rc;
+
+    int first_err = GCM_OK;
+    std::vector<uint32_t> small[2], large;                  // small[0]: AES-128, small[1]: AES-256
+    for (uint32_t i = 0; i < n; i++) {
+        gcm_msg &m = msgs[i];
+        m.status = check_msg(m);
+        if (m.status != GCM_OK) { if (first_err == GCM_OK) first_err = m.status; continue; }
+        BatchDesc &d = g.h_desc[i];
+        memset(&d, 0, sizeof(d));
+        memcpy(d.key, m.key, m.key_bits / 8);
+        memcpy(d.iv, m.iv, 12);
+        if (decrypt) memcpy(d.tag, m.tag, 16);
+        d.aad = (const uint8_t *)m.d_aad; d.in = (const uint8_t *)m.d_in; d.out = (uint8_t *)m.d_out;
+        d.aad_len = m.aad_len; d.len = m.len;
+        if (m.len >= BATCH_LARGE_BYTES) large.push_back(i);
+        else small[m.key_bits == 256].push_back(i);
+    }
+    // longest first: the tail of the ticket queue is then made of short messages
+    uint32_t pos = 0, start[2], count[2];
+    for (int k = 0; k < 2; k++) {
+        std::stable_sort(small[k].begin(), small[k].end(),
+                         [&](uint32_t a, uint32_t b) { return msgs[a].len > msgs[b].len; });
+        start[k] = pos; count[k] = (uint32_t)small[k].size();
+        for (uint32_t i : small[k]) g.h_order[pos++] = i;
+    }
+    CUB(cudaMemcpyAsync(g.d_desc, g.h_desc, (size_t)n * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
+    if (pos) CUB(cudaMemcpyAsync(g.d_order, g.h_order, (size_t)pos * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
+    CUB(cudaMemsetAsync(g.d_next, 0, 2 * sizeof(unsigned), s));
+    CUB(cudaMemsetAsync(g.d_res, 0, (size_t)n * sizeof(BatchResult), s));
+    for (int k = 0; k < 2; k++) {
+        if (!count[k]) continue;
+        const uint32_t want = (count[k] + BATCH_WARPS - 1) / BATCH_WARPS;
+        const int blocks = (int)std::min<uint32_t>(want, (uint32_t)g.sm_count);
+        cudaError_t e;
+        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s)
+                                : launch_batch<10, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s);
+        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s)
+                                : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s);
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+    }
+    for (uint32_t i : large) {
+        gcm_msg &m = msgs[i];
+        gcm_ctx *c = nullptr;
+        rc = ctx_for_key_locked(m.key, m.key_bits, s, &c);
+        if (rc == GCM_OK) {
+            rc = decrypt ? gcm_decrypt_verify_async(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out,
+                                                    g.d_desc[i].tag, &g.d_res[i].status, s)
+                         : gcm_encrypt_async(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out, g.d_res[i].tag, s);
+        }
+        if (rc != GCM_OK) { m.status = rc; if (first_err == GCM_OK) first_err = rc; }
+    }
+    CUB(cudaMemcpyAsync(g.h_res, g.d_res, (size_t)n * sizeof(BatchResult), cudaMemcpyDeviceToHost, s));
+    // the descriptors hold raw keys: wipe the device copy on the stream, the host copy after the sync
+    launch_wipe((uint8_t *)g.d_desc, (uint64_t)n * sizeof(BatchDesc), nullptr, s);
+    CUB(cudaGetLastError());
+    CUB(cudaStreamSynchronize(s));
+    secure_zero(g.h_desc, (size_t)n * sizeof(BatchDesc));
+    int failures = 0;
+    for (uint32_t i = 0; i < n; i++) {
+        gcm_msg &m = msgs[i];
+        if (m.status != GCM_OK) continue;
+        if (decrypt) {
+            m.status = g.h_res[i].status != 0 ? GCM_ERR_AUTH : GCM_OK;
+            if (m.status == GCM_ERR_AUTH) failures++;
+        } else {
+            memcpy(m.tag, g.h_res[i].tag, 16);
+        }
+    }
+    if (first_err != GCM_OK) return first_err;
+    return decrypt ? failures : GCM_OK;
+}
+
 }  // namespace
 
 extern "C" void gcm_batch_release(void)
 {
-    std::lock_guard<std::mutex> lock(g_cache.mu);
-    evict_all_locked();
-}
-
-static int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
-{
-    if (n && !msgs) return GCM_ERR_ARG;
-    std::lock_guard<std::mutex> lock(g_cache.mu);
-    int first_err = GCM_OK, failures = 0;
-    for (uint32_t i = 0; i < n; i++) {
-        gcm_msg &m = msgs[i];
-        gcm_ctx *c = nullptr;
-        int rc = ctx_for_key(m.key, m.key_bits, &c);
-        if (rc == GCM_OK) {
-            rc = decrypt ? gcm_decrypt_verify(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out, m.tag, stream)
-                         : gcm_encrypt(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out, m.tag, stream);
-        }
-        m.status = rc;
-        if (rc < 0 && first_err == GCM_OK) first_err = rc;
-        if (rc == GCM_ERR_AUTH) failures++;
-    }
-    if (first_err != GCM_OK) return first_err;
-    return decrypt ? failures : GCM_OK;
+    std::lock_guard<std::mutex> lock(g.mu);
+    evict_keys_locked();
+    free_staging_locked();
 }
 
 extern "C" int gcm_encrypt_batch(gcm_msg *msgs, uint32_t n, void *stream) { return run_batch(msgs, n, stream, false); }

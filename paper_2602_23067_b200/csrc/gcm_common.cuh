@@ -57,7 +57,6 @@ struct GcmTables {
 // pad (0..31) is chosen so that counter = virtual index + ctr_delta with ctr_delta = 0 mod 32.
 struct GcmParams {
     uint32_t rk[60];         // round keys, little-endian column words: rk[4r + c]
-    uint32_t iv_rk0[3];      // IV words ^ rk[0..2]: columns 0..2 of every counter block after AddRoundKey(0)
     uint32_t iv[3];          // IV words (little-endian load of bytes 0..11)
     const uint8_t *in;
     uint8_t       *out;

@@ -28,179 +28,7 @@
 #include "gf128.cuh"
 #include "gcm_fused.cuh"
 
-__device__ __forceinline__ uint32_t lds32(const uint8_t *sm, uint32_t off)
-{
-    return *reinterpret_cast<const uint32_t *>(sm + off);
-}
-__device__ __forceinline__ uint4 lds128(const uint8_t *sm, uint32_t off)
-{
-    return *reinterpret_cast<const uint4 *>(sm + off);
-}
-__device__ __forceinline__ uint32_t rotl32(uint32_t x, int n) { return __funnelshift_l(x, x, n); }
-
-// byte address of row (state byte `row` of w) in this lane's bank column: one PRMT
-#define TIDX(w, row) __byte_perm((w), lane4, 0x5504u | ((row) << 4))
-
-// Round-1 contribution of the three constant columns of a counter block (IV words ^ rk[0..2]):
-// twelve of the sixteen round-1 table reads do not depend on the counter and are done once per thread.
-struct CtrConst { uint32_t c0, c1, c2, c3; };
-
-__device__ __forceinline__ CtrConst ctr_const(const GcmParams &p, const uint8_t *sm, uint32_t lane4)
-{
-    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
-    const uint32_t s0 = p.iv_rk0[0], s1 = p.iv_rk0[1], s2 = p.iv_rk0[2];
-    CtrConst c;
-    c.c0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ p.rk[4];
-    c.c1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[5];
-    c.c2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[6];
-    c.c3 = lds32(sm, TIDX(s0, 1) + T1) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[7];
-    return c;
-}
-
-// Rounds 1-2 state that depends only on the upper 24 counter bits (see the header): the parts of the
-// four round-2 output columns that do not come from round-1 column 0.
-struct CtrCache { uint32_t u0, u1, u2, u3; };
-
-__device__ __forceinline__ CtrCache ctr_cache(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
-                                              const CtrConst &cc, uint32_t ctr)
-{
-    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
-    const uint32_t c3 = bswap32(ctr) ^ p.rk[3];
-    const uint32_t s1 = cc.c1 ^ lds32(sm, TIDX(c3, 2) + T2);
-    const uint32_t s2 = cc.c2 ^ lds32(sm, TIDX(c3, 1) + T1);
-    const uint32_t s3 = cc.c3 ^ lds32(sm, TIDX(c3, 0) + T0);
-    CtrCache u;
-    u.u0 = lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[8];
-    u.u1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ p.rk[9];
-    u.u2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[10];
-    u.u3 = lds32(sm, TIDX(s3, 0) + T0) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[11];
-    return u;
-}
-
-// E_K(IV || BE32(ctr)): a4 + a5.  Little-endian column words; the counter sits in column 3.  `u`
-// must have been made by ctr_cache() from a counter with the same upper 24 bits.
-template <int NR>
-__device__ __forceinline__ uint4 aes_ctr_block(const GcmParams &p, const uint8_t *sm, uint32_t lane4,
-                                               const CtrConst &cc, const CtrCache &u, uint32_t ctr)
-{
-    constexpr uint32_t T0 = AES_A0_OFF, T1 = AES_A0_OFF + AES_ODD_OFF, T2 = AES_A1_OFF, T3 = AES_A1_OFF + AES_ODD_OFF;
-    // round 1: only column 0 depends on the low counter byte (state byte 15 = byte 3 of column 3)
-    const uint32_t c3 = (ctr << 24) ^ p.rk[3];
-    const uint32_t r0 = cc.c0 ^ lds32(sm, TIDX(c3, 3) + T3);
-    // round 2: one read per column is indexed by round-1 column 0
-    uint32_t s0 = u.u0 ^ lds32(sm, TIDX(r0, 0) + T0);
-    uint32_t s1 = u.u1 ^ lds32(sm, TIDX(r0, 3) + T3);
-    uint32_t s2 = u.u2 ^ lds32(sm, TIDX(r0, 2) + T2);
-    uint32_t s3 = u.u3 ^ lds32(sm, TIDX(r0, 1) + T1);
-#pragma unroll
-    for (int r = 3; r < NR; r++) {
-        uint32_t t0 = lds32(sm, TIDX(s0, 0) + T0) ^ lds32(sm, TIDX(s1, 1) + T1) ^ lds32(sm, TIDX(s2, 2) + T2) ^ lds32(sm, TIDX(s3, 3) + T3) ^ p.rk[4 * r + 0];
-        uint32_t t1 = lds32(sm, TIDX(s1, 0) + T0) ^ lds32(sm, TIDX(s2, 1) + T1) ^ lds32(sm, TIDX(s3, 2) + T2) ^ lds32(sm, TIDX(s0, 3) + T3) ^ p.rk[4 * r + 1];
-        uint32_t t2 = lds32(sm, TIDX(s2, 0) + T0) ^ lds32(sm, TIDX(s3, 1) + T1) ^ lds32(sm, TIDX(s0, 2) + T2) ^ lds32(sm, TIDX(s1, 3) + T3) ^ p.rk[4 * r + 2];
-        uint32_t t3 = lds32(sm, TIDX(s3, 0) + T0) ^ lds32(sm, TIDX(s0, 1) + T1) ^ lds32(sm, TIDX(s1, 2) + T2) ^ lds32(sm, TIDX(s2, 3) + T3) ^ p.rk[4 * r + 3];
-        s0 = t0; s1 = t1; s2 = t2; s3 = t3;
-    }
-    // Final round (no MixColumns): S(x) sits in byte 0 of T2[x], bytes 1 and 2 of T0[x], byte 3 of T1[x].
-    uint4 o;
-#define FINAL(a, b, c, d, k)                                                                       \
-    (__byte_perm(__byte_perm(lds32(sm, TIDX(a, 0) + T2), lds32(sm, TIDX(b, 1) + T0), 0x0050),      \
-                 __byte_perm(lds32(sm, TIDX(c, 2) + T0), lds32(sm, TIDX(d, 3) + T1), 0x7200), 0x7610) ^ p.rk[4 * NR + (k)])
-    o.x = FINAL(s0, s1, s2, s3, 0);
-    o.y = FINAL(s1, s2, s3, s0, 1);
-    o.z = FINAL(s2, s3, s0, s1, 2);
-    o.w = FINAL(s3, s0, s1, s2, 3);
-#undef FINAL
-    return o;
-}
-
-// y . K for the fixed stride power K: sixteen 16-byte table entries XORed (a7).  sel[r] =
-// ((lane + r) & 7) << 4 is both the PRMT selector that moves byte (lane + r) & 7 of the 8-byte half
-// into address byte 1 and the 16-byte column offset of that position inside the 128-byte half-row.
-__device__ __forceinline__ uint4 ghash_mul_k(const uint8_t *sm, const uint32_t (&sel)[8], uint4 y)
-{
-    uint4 acc = make_uint4(0, 0, 0, 0);
-#pragma unroll
-    for (int r = 0; r < 8; r++) {
-        uint32_t off = (__byte_perm(y.x, y.y, sel[r]) & 0xFF00u) | sel[r];
-        acc = xor4(acc, lds128(sm, KTAB_OFF + off));
-    }
-#pragma unroll
-    for (int r = 0; r < 8; r++) {
-        uint32_t off = (__byte_perm(y.z, y.w, sel[r]) & 0xFF00u) | sel[r];
-        acc = xor4(acc, lds128(sm, KTAB_OFF + 128 + off));
-    }
-    return acc;
-}
-
-__device__ __forceinline__ uint4 ld16_stream(const uint8_t *p)
-{
-    return __ldcs(reinterpret_cast<const uint4 *>(p));
-}
-__device__ __forceinline__ void st16_stream(uint8_t *p, uint4 v)
-{
-    __stcs(reinterpret_cast<uint4 *>(p), v);
-}
-
-// n (0..16) bytes -> block, zero-padded (a ragged tail, an unaligned buffer, an AAD block)
-static __device__ __noinline__ uint4 load_bytes(const uint8_t *p, uint32_t n)
-{
-    uint32_t w[4] = {0, 0, 0, 0};
-    for (uint32_t i = 0; i < n; i++) w[i >> 2] |= (uint32_t)p[i] << (8 * (i & 3));
-    return make_uint4(w[0], w[1], w[2], w[3]);
-}
-static __device__ __noinline__ void store_bytes(uint8_t *p, uint4 v, uint32_t n)
-{
-    uint32_t w[4] = {v.x, v.y, v.z, v.w};
-    for (uint32_t i = 0; i < n; i++) p[i] = (uint8_t)(w[i >> 2] >> (8 * (i & 3)));
-}
-// keep the first n bytes, zero the rest (GHASH sees the ciphertext zero-padded, never keystream)
-__device__ __forceinline__ uint4 keep_bytes(uint4 v, uint32_t n)
-{
-    uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        int nb = (int)n - 4 * k;
-        uint32_t m = nb >= 4 ? 0xFFFFFFFFu : (nb <= 0 ? 0u : ((1u << (8 * nb)) - 1u));
-        w[k] &= m;
-    }
-    return make_uint4(w[0], w[1], w[2], w[3]);
-}
-
-// XOR of v over the CTA; result valid in thread 0.  red: 32 x uint4 of shared memory.
-__device__ __forceinline__ uint4 cta_xor_reduce(uint4 v, uint4 *red)
-{
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) {
-        v.x ^= __shfl_xor_sync(0xFFFFFFFFu, v.x, o); v.y ^= __shfl_xor_sync(0xFFFFFFFFu, v.y, o);
-        v.z ^= __shfl_xor_sync(0xFFFFFFFFu, v.z, o); v.w ^= __shfl_xor_sync(0xFFFFFFFFu, v.w, o);
-    }
-    if (lane == 0) red[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        v = lane < nwarps ? red[lane] : make_uint4(0, 0, 0, 0);
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) {
-            v.x ^= __shfl_xor_sync(0xFFFFFFFFu, v.x, o); v.y ^= __shfl_xor_sync(0xFFFFFFFFu, v.y, o);
-            v.z ^= __shfl_xor_sync(0xFFFFFFFFu, v.z, o); v.w ^= __shfl_xor_sync(0xFFFFFFFFu, v.w, o);
-        }
-    }
-    __syncthreads();
-    return v;
-}
-
-template <int TPB>
-__device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const uint32_t *te0)
-{
-    uint32_t *a0 = reinterpret_cast<uint32_t *>(sm + AES_A0_OFF);
-    uint32_t *a1 = reinterpret_cast<uint32_t *>(sm + AES_A1_OFF);
-    for (uint32_t j = threadIdx.x; j < 16384; j += TPB) {
-        uint32_t te = __ldg(te0 + (j >> 6));
-        bool odd = (j >> 5) & 1;
-        a0[j] = odd ? rotl32(te, 8) : te;            // T0 | T1
-        a1[j] = odd ? rotl32(te, 24) : rotl32(te, 16); // T2 | T3
-    }
-}
+#include "gcm_device.cuh"
 
 // H^d for d < 2^36 from the radix-512 digit table: four factors, two multiply levels, every lane
 // of the warp takes part (lane & 3 picks the digit) and ends up with the product.
@@ -255,7 +83,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
     CtrConst cc = {0, 0, 0, 0};
     CtrCache cu = {0, 0, 0, 0};
-    if (MODE != MODE_GHASH) cc = ctr_const(p, sm, lane4);
+    if (MODE != MODE_GHASH) cc = ctr_const(p.rk, p.iv[0], p.iv[1], p.iv[2], sm, lane4);
 
     uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
@@ -297,8 +125,8 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             // a4: counter from the virtual index alone; the upper 24 bits are warp-uniform and change
             // every 8th row, when rounds 1-2 are re-cached
             const uint32_t ctr = (uint32_t)v + p.ctr_delta;
-            if (row == r0 || (ctr & 0xE0u) == 0) cu = ctr_cache(p, sm, lane4, cc, ctr);
-            const uint4 ks = aes_ctr_block<NR>(p, sm, lane4, cc, cu, ctr);     // a5
+            if (row == r0 || (ctr & 0xE0u) == 0) cu = ctr_cache(p.rk, sm, lane4, cc, ctr);
+            const uint4 ks = aes_ctr_block<NR>(p.rk, sm, lane4, cc, cu, ctr);     // a5
             const uint4 y = xor4(x, ks);                                   // a6
             if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
             else if (cbytes) store_bytes(p.out + 16 * g, y, cbytes);
@@ -361,8 +189,8 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             *p.tag_out = Sg;
         } else {
             // a3 + a11: E_K(J0), J0 = IV || 0^31 || 1; tag; constant-time compare
-            cu = ctr_cache(p, sm, lane4, cc, 1u);
-            const uint4 ek = aes_ctr_block<NR>(p, sm, lane4, cc, cu, 1u);
+            cu = ctr_cache(p.rk, sm, lane4, cc, 1u);
+            const uint4 ek = aes_ctr_block<NR>(p.rk, sm, lane4, cc, cu, 1u);
             const uint4 tag = xor4(Sg, ek);
             if (MODE == MODE_ENCRYPT) {
                 *p.tag_out = tag;

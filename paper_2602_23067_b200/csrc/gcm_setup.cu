@@ -180,7 +180,16 @@ __global__ void gcm_wipe_kernel(uint8_t *dst, uint64_t len, const int *status)
     for (uint64_t k = head + mid * 16 + i; k < len; k += stride) dst[k] = 0;
 }
 
+// The key-independent round table alone (the batched kernel expands its keys itself).
+__global__ void gcm_te0_kernel(uint32_t *te0)
+{
+    const uint32_t t = threadIdx.x;
+    const uint32_t s = sbox_of(t), s2 = gf8_xtime(s), s3 = s2 ^ s;
+    te0[t] = s2 | (s << 8) | (s << 16) | (s3 << 24);
+}
+
 void launch_setup(const SetupParams &p, cudaStream_t s) { gcm_setup_kernel<<<1, 512, 0, s>>>(p); }
+void launch_te0(uint32_t *te0, cudaStream_t s) { gcm_te0_kernel<<<1, 256, 0, s>>>(te0); }
 void launch_wipe(uint8_t *dst, uint64_t len, const int *status, cudaStream_t s)
 {
     if (len == 0) return;

@@ -17,4 +17,5 @@ struct SetupParams {
 __device__ void gcm_build_power_tables(uint4 h, uint4 *hpow, uint4 *hx, uint4 *ktab, uint4 *s_v);
 
 void launch_setup(const SetupParams &p, cudaStream_t s);
+void launch_te0(uint32_t *te0, cudaStream_t s);
 void launch_wipe(uint8_t *dst, uint64_t len, const int *status, cudaStream_t s);

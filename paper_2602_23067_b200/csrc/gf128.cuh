@@ -91,19 +91,8 @@ __device__ __forceinline__ void clmul64(uint32_t xh, uint32_t xl, uint32_t yh, u
 // and the lower 128 bits the canon form of (degrees 128..254) / x^128, which is folded back with
 // x^128 = 1 + x + x^2 + x^7 (multiplying by x^s is a right shift by s; the up to 7 bits that fall off
 // are folded once more and then fit).  ~350 ALU + 144 IMAD.WIDE instructions, short dependency chains.
-static __device__ __noinline__ gf128 gf_mul(gf128 a, gf128 b)
+__device__ __forceinline__ gf128 gf_reduce256(const uint32_t (&p)[8])     // p[0] least significant
 {
-    uint32_t hh[4], ll[4], mm[4];
-    clmul64(a.w[0], a.w[1], b.w[0], b.w[1], hh);
-    clmul64(a.w[2], a.w[3], b.w[2], b.w[3], ll);
-    clmul64(a.w[0] ^ a.w[2], a.w[1] ^ a.w[3], b.w[0] ^ b.w[2], b.w[1] ^ b.w[3], mm);
-    uint32_t p[8];                                     // p[0] least significant
-    p[0] = ll[0]; p[1] = ll[1];
-    p[2] = ll[2] ^ mm[0] ^ hh[0] ^ ll[0];
-    p[3] = ll[3] ^ mm[1] ^ hh[1] ^ ll[1];
-    p[4] = hh[0] ^ mm[2] ^ hh[2] ^ ll[2];
-    p[5] = hh[1] ^ mm[3] ^ hh[3] ^ ll[3];
-    p[6] = hh[2]; p[7] = hh[3];
     // P << 1
     const uint32_t lo0 = __funnelshift_l(p[6], p[7], 1), lo1 = __funnelshift_l(p[5], p[6], 1);
     const uint32_t lo2 = __funnelshift_l(p[4], p[5], 1), lo3 = __funnelshift_l(p[3], p[4], 1);
@@ -118,6 +107,46 @@ static __device__ __noinline__ gf128 gf_mul(gf128 a, gf128 b)
     r.w[2] = lo2 ^ h2 ^ __funnelshift_r(h2, h1, 1) ^ __funnelshift_r(h2, h1, 2) ^ __funnelshift_r(h2, h1, 7);
     r.w[3] = lo3 ^ h3 ^ __funnelshift_r(h3, h2, 1) ^ __funnelshift_r(h3, h2, 2) ^ __funnelshift_r(h3, h2, 7);
     return r;
+}
+
+static __device__ __noinline__ gf128 gf_mul(gf128 a, gf128 b)
+{
+    uint32_t hh[4], ll[4], mm[4];
+    clmul64(a.w[0], a.w[1], b.w[0], b.w[1], hh);
+    clmul64(a.w[2], a.w[3], b.w[2], b.w[3], ll);
+    clmul64(a.w[0] ^ a.w[2], a.w[1] ^ a.w[3], b.w[0] ^ b.w[2], b.w[1] ^ b.w[3], mm);
+    uint32_t p[8];                                     // p[0] least significant
+    p[0] = ll[0]; p[1] = ll[1];
+    p[2] = ll[2] ^ mm[0] ^ hh[0] ^ ll[0];
+    p[3] = ll[3] ^ mm[1] ^ hh[1] ^ ll[1];
+    p[4] = hh[0] ^ mm[2] ^ hh[2] ^ ll[2];
+    p[5] = hh[1] ^ mm[3] ^ hh[3] ^ ll[3];
+    p[6] = hh[2]; p[7] = hh[3];
+    return gf_reduce256(p);
+}
+
+// a . a: squaring over GF(2) only spreads the bits (bit j of the integer moves to bit 2j), then the
+// same reduction.  Used for the H^(2^k) ladder of PAPER.md L197.
+__device__ __forceinline__ uint64_t spread32(uint32_t x)
+{
+    uint64_t t = x;
+    t = (t | (t << 16)) & 0x0000FFFF0000FFFFull;
+    t = (t | (t << 8)) & 0x00FF00FF00FF00FFull;
+    t = (t | (t << 4)) & 0x0F0F0F0F0F0F0F0Full;
+    t = (t | (t << 2)) & 0x3333333333333333ull;
+    t = (t | (t << 1)) & 0x5555555555555555ull;
+    return t;
+}
+static __device__ __noinline__ gf128 gf_sqr(gf128 a)
+{
+    uint32_t p[8];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {                      // a.w[3] is the least significant word
+        const uint64_t t = spread32(a.w[3 - i]);
+        p[2 * i] = (uint32_t)t;
+        p[2 * i + 1] = (uint32_t)(t >> 32);
+    }
+    return gf_reduce256(p);
 }
 
 __device__ __forceinline__ uint4 xor4(uint4 a, uint4 b)

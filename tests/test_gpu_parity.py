@@ -298,6 +298,75 @@ def test_config_c4_scaled_batch(G, oracle):
     G.gcm_batch_release()
 
 
+def test_batch_warp_per_message_kernel(G, oracle):
+    """The one-warp-per-message kernel: both key sizes in one call, every tail shape, empty messages,
+    empty AAD, unaligned buffers, messages packed in one buffer at 16-byte offsets (config C4's layout),
+    then decrypt_verify with a few tampered messages: rejected, zero-filled, neighbours untouched."""
+    rng = np.random.default_rng(9650)
+    lens = [0, 1, 15, 16, 17, 31, 32, 33, 495, 496, 497, 511, 512, 513, 1023, 1024, 4096, 8191, 8192 + 5,
+            16 * 32 * 7, 16 * 32 * 7 + 16 * 30, 16 * 32 * 7 + 16 * 30 + 9, 65536, 70001, 200000]
+    lens += rng.integers(1, 65537, 40).tolist()
+    specs = []
+    for i, n in enumerate(lens):
+        klen = 16 if i % 3 else 32
+        a = [0, 1, 16, 17, 100, 256, 2880][i % 7]
+        specs.append((rnd(rng, klen).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, a), rnd(rng, n), i % 5 == 4))
+    # one packed buffer; unaligned messages start 3 bytes past a 16-byte boundary
+    offs, pos = [], 0
+    for (_, _, _, pt, unal) in specs:
+        pos = (pos + 15) // 16 * 16 + (3 if unal else 0)
+        offs.append(pos)
+        pos += len(pt) + 16            # a guard gap after every message
+    big_in = torch.zeros(pos + 16, dtype=torch.uint8, device="cuda")
+    big_out = torch.zeros(pos + 16, dtype=torch.uint8, device="cuda")
+    for (_, _, _, pt, _), o in zip(specs, offs):
+        if len(pt):
+            big_in[o: o + len(pt)] = dev(pt)
+    batch = []
+    for (key, iv, aad, pt, _), o in zip(specs, offs):
+        batch.append({"key": key, "iv": iv, "aad": dev(aad) if len(aad) else None,
+                      "input": big_in[o: o + len(pt)], "output": big_out[o: o + len(pt)]})
+    tags = G.gcm_encrypt_batch(batch)
+    out = big_out.cpu().numpy()
+    covered = np.zeros(out.size, bool)
+    for (key, iv, aad, pt, _), o, tag in zip(specs, offs, tags):
+        ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+        assert tag == ref_tag, "tag len=%d aad=%d" % (len(pt), len(aad))
+        assert np.array_equal(out[o: o + len(pt)], ref_ct), "ct len=%d aad=%d" % (len(pt), len(aad))
+        covered[o: o + len(pt)] = True
+    assert not out[~covered].any(), "wrote outside a message's output range"
+    # decrypt: tamper message 5 (tag), 9 (ciphertext), 20 (aad), 24 (last byte of a 200000-byte message)
+    dec_out = torch.full_like(big_out, 0x77)
+    dec = []
+    for i, (b, tag) in enumerate(zip(batch, tags)):
+        o, n = offs[i], len(specs[i][3])
+        dec.append({"key": b["key"], "iv": b["iv"], "aad": b["aad"], "input": big_out[o: o + n],
+                    "output": dec_out[o: o + n], "tag": tag})
+    bad = {5, 9, 20, 24}
+    t = bytearray(tags[5]); t[15] ^= 1; dec[5]["tag"] = bytes(t)
+    big_out[offs[9] + len(specs[9][3]) // 2] ^= 0x10
+    a20 = dec[20]["aad"].clone(); a20[0] ^= 0x80; dec[20]["aad"] = a20
+    big_out[offs[24] + len(specs[24][3]) - 1] ^= 1
+    st = G.gcm_decrypt_verify_batch(dec)
+    got = dec_out.cpu().numpy()
+    for i, (spec, o) in enumerate(zip(specs, offs)):
+        n = len(spec[3])
+        if i in bad:
+            assert st[i] == G.GCM_ERR_AUTH, i
+            assert not got[o: o + n].any(), "message %d not suppressed" % i
+        else:
+            assert st[i] == G.GCM_OK, i
+            assert np.array_equal(got[o: o + n], spec[3]), i
+    assert (got[~covered] == 0x77).all()
+    # argument errors are reported per message and do not stop the others
+    batch2 = [dict(batch[1]), dict(batch[2])]
+    batch2[0]["key"] = bytes(24)
+    with pytest.raises(G.GcmError) as e:
+        G.gcm_encrypt_batch(batch2)
+    assert e.value.code == G.GCM_ERR_ARG
+    G.gcm_batch_release()
+
+
 def test_host_buffers_single_chunk(G, oracle):
     rng = np.random.default_rng(9700)
     key = rnd(rng, 32).tobytes()
