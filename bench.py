@@ -49,7 +49,10 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sample-mib", type=float, default=48.0)
+    ap.add_argument("--cpu-sample-mib", type=float, default=384.0)
+    ap.add_argument("--workload", default="c5",
+                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency"],
+                    help="c5 = the headline (default); the others are the supplementary measurements of DESIGN.md section 10")
     return ap.parse_args()
 
 
@@ -122,13 +125,14 @@ def measured_peaks() -> dict:
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
 
 
-def pipe_bound_gbs(nr: int, sm_count: int, sm_mhz: float) -> dict:
+def pipe_bound_gbs(nr: int, sm_count: int, sm_mhz: float, mode: str = "enc") -> dict:
     """Shared-memory-pipe bound of the method.  Per 16-byte block the path needs
     16*nr conflict-free 4-byte AES table reads minus the ones that do not depend on the low counter
     byte (12 round-1 reads of the constant IV columns, hoisted per thread; 3 round-1 + 12 round-2
     reads cached per lane and refreshed every 8th block: -27 + 15/8), plus 16 16-byte GHASH table
-    reads = 64 bank-lanes; an SM serves 32 bank-lanes (one 128-byte wavefront) per cycle."""
-    lanes = 16 * nr - 27 + 15.0 / 8.0 + 64
+    reads = 64 bank-lanes; an SM serves 32 bank-lanes (one 128-byte wavefront) per cycle.
+    mode "ghash": the GHASH table reads alone."""
+    lanes = 64.0 if mode == "ghash" else 16 * nr - 27 + 15.0 / 8.0 + 64
     cycles = lanes / 32.0
     return {"lanes_per_block": lanes, "cycles_per_block_per_sm": cycles,
             "gbs": sm_count * sm_mhz * 1e6 * 16.0 / cycles / 1e9}
@@ -347,12 +351,178 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------------
+# supplementary measurements: same timing rules, one JSON line each
+# ---------------------------------------------------------------------------------------------------
+def run_extra(args):
+    import numpy as np
+    import torch
+    import paper_2602_23067_b200 as G
+    import workloads
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    G.gcm_set_device(0)
+    stream = torch.cuda.current_stream()
+    peaks = measured_peaks()
+    sm_count = torch.cuda.get_device_properties(0).multi_processor_count
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    w = args.workload
+    steps, warm = args.steps, max(3, args.warmup)
+
+    def timed(step):
+        for _ in range(warm):
+            step()
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        sampler = ClockSampler(0)
+        sampler.start()
+        ev[0].record(stream)
+        for i in range(steps):
+            step()
+            ev[i + 1].record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        per = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+        return ev[0].elapsed_time(ev[-1]), per, clocks
+
+    def rand_bytes(n, seed):
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(seed)
+        return torch.randint(-2 ** 63, 2 ** 63 - 1, ((n + 7) // 8,), dtype=torch.int64, device="cuda",
+                             generator=gen).view(torch.uint8)[:n]
+
+    line = {"unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warm, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic", "supplementary": True}
+
+    if w in ("c5-decrypt", "c5-ghash", "c5-aes128", "c2"):
+        n = (256 << 20) if w == "c2" else int(args.size_mib * (1 << 20))
+        m = workloads.config_c2(payload_bytes=0) if w == "c2" else workloads.config_c5(payload_bytes=n, with_payload=False)
+        key = m.key[:16] if w == "c5-aes128" else m.key
+        nr = 10 if len(key) == 16 else 14
+        pt = rand_bytes(n, workloads.SEEDS["C2" if w == "c2" else "C5"])
+        ct = torch.empty(n, dtype=torch.uint8, device="cuda")
+        aad = torch.from_numpy(m.aad).cuda()
+        d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        d_status = torch.zeros(1, dtype=torch.int32, device="cuda")
+        ctx = G.gcm_init(key)
+        G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+        if w == "c5-decrypt":
+            back = torch.empty(n, dtype=torch.uint8, device="cuda")
+            step = lambda: G.gcm_decrypt_verify_async(ctx, m.iv, aad, ct, back, d_tag, d_status, stream)
+            launches, mode, what = 2, "enc", "AES-256-GCM decrypt_verify (fused kernel + gated wipe kernel)"
+        elif w == "c5-ghash":
+            d_s = torch.zeros(16, dtype=torch.uint8, device="cuda")
+            step = lambda: G.gcm_ghash_async(ctx, aad, ct, d_s, stream)
+            launches, mode, what = 1, "ghash", "GHASH only over device-resident ciphertext (the paper's Table 5 scope, L363)"
+        else:
+            step = lambda: G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+            launches, mode, what = 1, "enc", "AES-%d-GCM encrypt" % (8 * len(key))
+        total_ms, per, clocks = timed(step)
+        if w == "c5-decrypt":
+            assert int(d_status.item()) == 0 and torch.equal(back[:1 << 20], pt[:1 << 20])
+        G.gcm_destroy(ctx)
+        gbs = steps * n / (total_ms * 1e-3) / 1e9
+        pb = pipe_bound_gbs(nr, sm_count, sm_mhz, mode)
+        line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
+                    config={"workload": "%s: %s, %d-byte message, 2880-byte AAD" % (w, what, n), "payload_bytes": n},
+                    gpu_launches=launches * steps, clocks=clocks,
+                    roofline={"bound": "alu", "pipe": "shared-memory wavefronts (LSU): %.1f bank-lanes per block" % pb["lanes_per_block"],
+                              "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"],
+                              "hbm_frac": (1 if mode == "ghash" else 2) * gbs / float(peaks["hbm_gbs"])},
+                    ms_per_step_median=statistics.median(per))
+    elif w == "c3":
+        msgs = workloads.config_c3()
+        batch = []
+        for m in msgs:
+            d_in = torch.from_numpy(m.payload).cuda()
+            batch.append({"key": m.key, "iv": m.iv, "aad": torch.from_numpy(m.aad).cuda(), "input": d_in,
+                          "output": torch.empty_like(d_in)})
+        nbytes = sum(m.payload.size for m in msgs)
+        total_ms, per, clocks = timed(lambda: G.gcm_encrypt_batch(batch, stream))
+        G.gcm_batch_release()
+        gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
+        pb = pipe_bound_gbs(14, sm_count, sm_mhz)
+        line.update(metric="AES-256-GCM batched encrypt GB/s (C3: 16 FITS images of 64 MiB)", value=gbs,
+                    ms_per_step=total_ms / steps, gpu_launches=(16 + 1) * steps, clocks=clocks,
+                    config={"workload": "c3: gcm_encrypt_batch, 16 x 67,109,760-byte FITS-shaped images, one AES-256 key, 16 IVs, "
+                                        "2880-byte header AAD each; synchronous call (descriptor upload, 16 fused launches, tag download inside)",
+                            "payload_bytes": nbytes},
+                    roofline={"bound": "alu", "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"]},
+                    ms_per_step_median=statistics.median(per))
+    elif w == "c4":
+        msgs = workloads.config_c4()
+        offs, total = [], 0
+        for m in msgs:
+            offs.append(total)
+            total += (m.payload.size + 15) // 16 * 16
+        h_in = np.zeros(total, np.uint8)
+        for m, o in zip(msgs, offs):
+            h_in[o: o + m.payload.size] = m.payload
+        d_in = torch.from_numpy(h_in).cuda()
+        d_out = torch.empty_like(d_in)
+        aads = [torch.from_numpy(m.aad).cuda() if m.aad.size else None for m in msgs]
+        batch = [{"key": m.key, "iv": m.iv, "aad": a, "input": d_in[o: o + m.payload.size],
+                  "output": d_out[o: o + m.payload.size]} for m, o, a in zip(msgs, offs, aads)]
+        nbytes = sum(m.payload.size for m in msgs)
+        # the binding's per-call marshalling of 10,000 Python dicts is host work outside the C ABI:
+        # marshal once, then time the C call itself
+        arr, cnt, keep = G.gcm._pack_msgs(batch, decrypt=False)
+        sp = G.gcm._stream(stream)
+
+        def step():
+            rc = G.gcm._L.gcm_encrypt_batch(arr, cnt, sp)
+            assert rc == 0
+        total_ms, per, clocks = timed(step)
+        G.gcm_batch_release()
+        gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
+        pb = pipe_bound_gbs(10, sm_count, sm_mhz)
+        line.update(metric="AES-128-GCM batched encrypt GB/s (C4: 10,000 messages of 1 B..64 KiB)", value=gbs,
+                    ms_per_step=total_ms / steps, gpu_launches=2 * steps, clocks=clocks,
+                    messages_per_s=steps * len(msgs) / (total_ms * 1e-3),
+                    config={"workload": "c4: gcm_encrypt_batch (C call), 10,000 AES-128 messages, len ~ U{1..65536}, AAD ~ U{0..256}, "
+                                        "own key and IV each, payloads packed at 16-byte-aligned offsets; synchronous call "
+                                        "(descriptor upload, one persistent warp-per-message kernel, tag download inside)",
+                            "payload_bytes": nbytes, "messages": len(msgs)},
+                    roofline={"bound": "alu", "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"],
+                              "note": "peak is the large-message bound of the 8-bit-table kernel; the per-message key schedule, "
+                                      "H ladder and 4-bit table build of this kernel are not in it"},
+                    ms_per_step_median=statistics.median(per))
+    elif w == "latency":
+        # single-message latency through the synchronous non-batched call (C4's report): host wall clock
+        m = workloads.config_c1(payload_bytes=0)
+        ctx = G.gcm_init(m.key)
+        aad = torch.from_numpy(m.aad).cuda()
+        out = {}
+        for n in (1024, 65536, 1 << 20):
+            pt = rand_bytes(n, 7 + n)
+            ct = torch.empty_like(pt)
+            for _ in range(50):
+                G.gcm_encrypt(ctx, m.iv, aad, pt, ct, stream)
+            ts = []
+            for _ in range(2000):
+                t0 = time.perf_counter()
+                G.gcm_encrypt(ctx, m.iv, aad, pt, ct, stream)
+                ts.append((time.perf_counter() - t0) * 1e6)
+            ts.sort()
+            out["%d_bytes" % n] = {"p50_us": ts[len(ts) // 2], "p99_us": ts[int(len(ts) * 0.99)], "min_us": ts[0]}
+        G.gcm_destroy(ctx)
+        line.update(metric="AES-128-GCM single-message latency through gcm_encrypt (us, host wall clock)", value=out["1024_bytes"]["p50_us"],
+                    unit="us", higher_is_better=False, ms_per_step=out["1024_bytes"]["p50_us"] / 1e3, gpu_launches=2000 * 3,
+                    config={"workload": "latency: synchronous gcm_encrypt of one 1 KiB / 64 KiB / 1 MiB AES-128 message, 16-byte AAD, 2000 calls each"},
+                    latency=out)
+    print(json.dumps(line))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
-    else:
+    elif args.workload == "c5":
         run_ours(args)
+    else:
+        run_extra(args)
 
 
 if __name__ == "__main__":
