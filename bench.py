@@ -205,25 +205,20 @@ def run_ours(args):
     import paper_2602_23067_b200 as G
     import workloads
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2602_23067_b200 import replicas
+    rank, local, world = replicas.rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
     G.gcm_set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
+    replicas.init("nccl", torch.device("cuda", local))
+    barrier = replicas.barrier
 
     n = int(args.size_mib * (1 << 20))
     m = workloads.config_c5(payload_bytes=n, with_payload=False)
-    key = bytes(x ^ rank for x in m.key) if rank else m.key      # one independent message per rank
+    key = replicas.replica_key(m.key, rank)                      # one independent message per rank
     gen = torch.Generator(device="cuda")
-    gen.manual_seed(workloads.SEEDS["C5"] + rank)
+    gen.manual_seed(replicas.replica_seed(workloads.SEEDS["C5"], rank))
     # uniform random bytes, generated on the device 8 bytes at a time
     pt = torch.randint(-2 ** 63, 2 ** 63 - 1, ((n + 7) // 8,), dtype=torch.int64, device="cuda", generator=gen).view(torch.uint8)[:n]
     ct = torch.empty(n, dtype=torch.uint8, device="cuda")
@@ -231,6 +226,7 @@ def run_ours(args):
     d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
     ctx = G.gcm_init(key)
     stream = torch.cuda.current_stream()
+    rates = G.gcm_measure_pipe_rates() if rank == 0 else {}   # unit rates behind the roofline (outside the timed region)
 
     def step():
         G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
@@ -266,11 +262,8 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else {}
     total_ms = ev[0].elapsed_time(ev[-1])
     per = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
-    value = world * args.steps * n / (total_ms * 1e-3) / 1e9
+    total_ms = replicas.max_over_ranks(total_ms, "cuda")
+    value = replicas.aggregate_gbs(n, args.steps, total_ms, world)
 
     # end to end: pinned host buffers through gcm_encrypt_host (H2D + kernels + D2H inside the region)
     e2e = None
@@ -287,21 +280,17 @@ def run_ours(args):
             tag_h = G.gcm_encrypt_host(ctx, m.iv, h_aad, h_pt, h_ct, stream)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
+        dt = replicas.max_over_ranks(dt, "cuda")
         assert tag_h == d_tag.cpu().numpy().tobytes(), "host-path tag differs from device-path tag"
         assert torch.equal(h_ct[:4096], ct[:4096].cpu()) and torch.equal(h_ct[-4096:], ct[-4096:].cpu())
-        e2e = {"value": world * args.e2e_steps * n / dt / 1e9, "unit": UNIT,
+        e2e = {"value": replicas.aggregate_gbs(n, args.e2e_steps, dt * 1e3, world), "unit": UNIT,
                "h2d_bytes_per_step": n + int(m.aad.size), "d2h_bytes_per_step": n + 16,
                "steps": args.e2e_steps, "how": "gcm_encrypt_host: pinned host in/out, chunked H2D -> fused kernel -> D2H"}
         del h_pt, h_ct
 
     G.gcm_destroy(ctx)
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        replicas.finish()
         return
 
     peaks = measured_peaks()
@@ -319,6 +308,8 @@ def run_ours(args):
         "algorithmic_bytes_per_launch": 2 * n,
         "hbm": {"achieved": 2 * achieved, "peak": hbm_peak, "unit": "GB/s", "frac": 2 * achieved / hbm_peak,
                 "of": peaks["_source"]},
+        "rates": {"unit": "thread-operations per SM-cycle, measured by gcm_measure_pipe_rates on this device",
+                  **{k: round(v, 2) for k, v in rates.items()}},
         "kernel": "gcm_fused_kernel<14, ENCRYPT, 512>", "kernel_ms_mean": kernel_ms,
         "kernel_ms_median": statistics.median(per),
     }
@@ -347,8 +338,7 @@ def run_ours(args):
         "ms_per_step_median": statistics.median(per), "ms_per_step_std": statistics.pstdev(per),
     }
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finish()
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -445,9 +435,9 @@ def run_extra(args):
         gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
         pb = pipe_bound_gbs(14, sm_count, sm_mhz)
         line.update(metric="AES-256-GCM batched encrypt GB/s (C3: 16 FITS images of 64 MiB)", value=gbs,
-                    ms_per_step=total_ms / steps, gpu_launches=(16 + 1) * steps, clocks=clocks,
+                    ms_per_step=total_ms / steps, gpu_launches=steps, clocks=clocks,
                     config={"workload": "c3: gcm_encrypt_batch, 16 x 67,109,760-byte FITS-shaped images, one AES-256 key, 16 IVs, "
-                                        "2880-byte header AAD each; synchronous call (descriptor upload, 16 fused launches, tag download inside)",
+                                        "2880-byte header AAD each; synchronous call (descriptor upload, ONE multi-message launch, tag download inside)",
                             "payload_bytes": nbytes},
                     roofline={"bound": "alu", "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"]},
                     ms_per_step_median=statistics.median(per))

@@ -88,6 +88,25 @@ GCM_API void gcm_destroy(gcm_ctx *ctx);
 GCM_API int gcm_set_geometry(gcm_ctx *ctx, int grid, int threads);
 GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
 
+/*
+ * Diagnostics for the roofline (the pipe bound must use MEASURED unit rates): runs
+ * a short probe on the current device and writes thread-operations per SM-cycle, averaged over the
+ * SMs, for the instruction classes the kernels are made of.  rates (host, out) has room for n >=
+ * GCM_RATE_COUNT doubles, indexed by the enum below.  Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
+ * Not part of the data path.
+ */
+enum {
+    GCM_RATE_LDS32 = 0,     /* conflict-free 4-byte shared-memory reads (the AES table read)        */
+    GCM_RATE_LDS128,        /* conflict-free 16-byte shared-memory reads (the GHASH table read)     */
+    GCM_RATE_LOP3,          /* three-input logic                                                     */
+    GCM_RATE_PRMT,          /* byte permute (table address formation)                                */
+    GCM_RATE_IMAD,          /* 32-bit integer multiply-add                                           */
+    GCM_RATE_IMAD_WIDE,     /* 32 x 32 + 64 -> 64 multiply-add (the generic GF(2^128) product)       */
+    GCM_RATE_LOP3_IMAD,     /* LOP3 and IMAD interleaved 1:1 (both pipes), operations of both kinds  */
+    GCM_RATE_COUNT
+};
+GCM_API int gcm_measure_pipe_rates(double *rates, int n);
+
 /* Copies the hash subkey H = E_K(0^128) (16 bytes) to host memory; for tests of step a2. */
 GCM_API int gcm_get_hash_subkey(const gcm_ctx *ctx, uint8_t h[16]);
 

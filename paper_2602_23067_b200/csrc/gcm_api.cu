@@ -44,10 +44,10 @@ extern "C" const char *gcm_last_cuda_error_string(void)
     return cudaGetErrorString((cudaError_t)g_last_cuda_error);
 }
 
-static void secure_zero(void *p, size_t n)
+static void secure_zero(void *p, size_t n)      // memset the compiler may not drop
 {
-    volatile uint8_t *v = (volatile uint8_t *)p;
-    while (n--) *v++ = 0;
+    memset(p, 0, n);
+    __asm__ __volatile__("" : : "r"(p) : "memory");
 }
 
 static SetupParams setup_params(gcm_ctx *c, const uint8_t *key)

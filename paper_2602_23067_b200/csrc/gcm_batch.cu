@@ -31,6 +31,7 @@
 #include "gcm_common.cuh"
 #include "gcm_device.cuh"
 #include "gcm_setup.cuh"
+#include "gcm_multi.cuh"
 #include "gcm_api_internal.h"
 
 #define BATCH_WARPS        12
@@ -60,6 +61,7 @@ struct BatchResult {          // one per message, device
     int status;
     int pad[3];
 };
+static_assert(sizeof(BatchResult) == sizeof(MultiResult), "BatchResult / MultiResult layout");
 
 // ---- device ---------------------------------------------------------------------------------------
 
@@ -289,13 +291,19 @@ struct BatchState {
     uint32_t *h_order = nullptr, *d_order = nullptr;
     unsigned *d_next = nullptr;      // [2]
     uint32_t *d_te0 = nullptr;
+    // staging of the large-message path (gcm_multi.cu): descriptors, chunks, per-warp chunk ranges,
+    // accumulators + tickets; one pinned block and one device block, grown on demand
+    uint8_t *h_multi = nullptr, *d_multi = nullptr;
+    size_t multi_cap = 0;
 };
 BatchState g;
 
+// memset that the compiler may not drop (the descriptor staging holds raw keys: 1 MB per 10,000 messages,
+// so this must run at memory speed, not byte by byte)
 void secure_zero(void *p, size_t n)
 {
-    volatile uint8_t *v = (volatile uint8_t *)p;
-    while (n--) *v++ = 0;
+    memset(p, 0, n);
+    __asm__ __volatile__("" : : "r"(p) : "memory");
 }
 
 void free_staging_locked()
@@ -310,6 +318,9 @@ void free_staging_locked()
     if (g.h_order) cudaFreeHost(g.h_order);
     if (g.d_next) cudaFree(g.d_next);
     if (g.d_te0) cudaFree(g.d_te0);
+    if (g.d_multi) cudaFree(g.d_multi);
+    if (g.h_multi) cudaFreeHost(g.h_multi);
+    g.d_multi = g.h_multi = nullptr; g.multi_cap = 0;
     g.d_desc = g.h_desc = nullptr; g.d_res = g.h_res = nullptr; g.d_order = g.h_order = nullptr;
     g.d_next = nullptr; g.d_te0 = nullptr; g.cap = 0; g.device = -1;
     cudaGetLastError();
@@ -361,16 +372,12 @@ int ensure_staging_locked(uint32_t n)
     return GCM_OK;
 }
 
-int ctx_for_key_locked(const uint8_t *key, int key_bits, cudaStream_t s, gcm_ctx **out)
+int ctx_for_key_locked(const uint8_t *key, int key_bits, gcm_ctx **out)
 {
     std::string id((const char *)key, key_bits / 8);
     id.push_back((char)g.device);
     auto it = g.by_key.find(id);
     if (it != g.by_key.end()) { *out = it->second; secure_zero(&id[0], id.size()); return GCM_OK; }
-    if (g.by_key.size() >= BatchState::kMaxKeys) {
-        cudaStreamSynchronize(s);          // queued launches may still use the contexts
-        evict_keys_locked();
-    }
     gcm_ctx *c = nullptr;
     int rc = gcm_init(&c, key, key_bits);
     if (rc == GCM_OK) { g.by_key[id] = c; *out = c; }
@@ -393,6 +400,127 @@ int check_msg(const gcm_msg &m)
         cudaError_t e__ = (call);                                                                  \
         if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
     } while (0)
+
+// Large messages (>= BATCH_LARGE_BYTES): grouped by key, ONE launch of gcm_multi_kernel per key (per-key
+// context cached across calls).  The rows of all messages of a group are dealt to the warps of the grid in
+// contiguous chunks of at most Q = ceil(total rows / warps) rows per warp.
+int run_large_locked(gcm_msg *msgs, const std::vector<uint32_t> &large, bool decrypt, cudaStream_t s, int *first_err)
+{
+    if (large.empty()) return GCM_OK;
+    struct Group { gcm_ctx *ctx; std::vector<uint32_t> idx; };
+    std::vector<Group> groups;
+    std::map<gcm_ctx *, size_t> where;
+    for (uint32_t i : large) {
+        gcm_ctx *c = nullptr;
+        int rc = ctx_for_key_locked(msgs[i].key, msgs[i].key_bits, &c);
+        if (rc == GCM_OK && (msgs[i].aad_len + 15) / 16 > 0xFFFFFFFFull) rc = GCM_ERR_LEN;
+        if (rc != GCM_OK) { msgs[i].status = rc; if (*first_err == GCM_OK) *first_err = rc; continue; }
+        auto it = where.find(c);
+        if (it == where.end()) { it = where.emplace(c, groups.size()).first; groups.push_back(Group{c, {}}); }
+        groups[it->second].idx.push_back(i);
+    }
+    if (groups.empty()) return GCM_OK;
+
+    const uint32_t W = (uint32_t)g.sm_count * (MULTI_THREADS / 32);
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    struct Layout { size_t msgs, chunks, wfirst, acc, counter; };
+    std::vector<Layout> lay(groups.size());
+    size_t total = 0;
+    for (size_t k = 0; k < groups.size(); k++) {
+        const size_t nk = groups[k].idx.size();
+        lay[k].msgs = total;    total += up(nk * sizeof(MultiMsg));
+        lay[k].chunks = total;  total += up((nk + W) * sizeof(MultiChunk));
+        lay[k].wfirst = total;  total += up((W + 1) * sizeof(uint32_t));
+        lay[k].acc = total;     total += up(nk * 16);
+        lay[k].counter = total; total += 256;
+    }
+    if (total > g.multi_cap) {
+        cudaStreamSynchronize(s);
+        if (g.d_multi) cudaFree(g.d_multi);
+        if (g.h_multi) cudaFreeHost(g.h_multi);
+        g.d_multi = g.h_multi = nullptr; g.multi_cap = 0;
+        size_t cap = 1 << 20;
+        while (cap < total) cap *= 2;
+        cudaError_t e = cudaHostAlloc((void **)&g.h_multi, cap, cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&g.d_multi, cap);
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+        g.multi_cap = cap;
+    }
+    memset(g.h_multi, 0, total);
+
+    for (size_t k = 0; k < groups.size(); k++) {
+        const std::vector<uint32_t> &idx = groups[k].idx;
+        MultiMsg *mm = (MultiMsg *)(g.h_multi + lay[k].msgs);
+        MultiChunk *ch = (MultiChunk *)(g.h_multi + lay[k].chunks);
+        uint32_t *wf = (uint32_t *)(g.h_multi + lay[k].wfirst);
+        uint64_t R = 0;
+        for (size_t j = 0; j < idx.size(); j++) {
+            const gcm_msg &m = msgs[idx[j]];
+            MultiMsg &d = mm[j];
+            memcpy(d.iv, m.iv, 12);
+            const uint64_t n_full = m.len / 16, n_blocks = (m.len + 15) / 16, n_aad = (m.aad_len + 15) / 16;
+            d.pad = (2u - (uint32_t)n_aad) & (GCM_STRIDE - 1);
+            d.in = (const uint8_t *)m.d_in; d.out = (uint8_t *)m.d_out; d.aad = (const uint8_t *)m.d_aad;
+            d.len = m.len; d.aad_len = m.aad_len;
+            d.base = (uint64_t)d.pad + n_aad;
+            d.vblocks = d.base + n_blocks;
+            d.n_aad_blocks = (uint32_t)n_aad;
+            d.rows = (uint32_t)((d.vblocks + GCM_STRIDE - 1) / GCM_STRIDE);
+            d.aligned = ((((uintptr_t)m.d_in) | ((uintptr_t)m.d_out)) & 15) == 0 ? 1u : 0u;
+            if (d.aligned) {
+                d.fast_lo = (uint32_t)((d.base + GCM_STRIDE - 1) / GCM_STRIDE);
+                d.fast_hi = (uint32_t)((d.base + n_full) / GCM_STRIDE);
+                if (d.fast_hi < d.fast_lo) d.fast_hi = d.fast_lo;
+            }
+            d.ctr_delta = 2u - (uint32_t)d.base;
+            if (decrypt) memcpy(d.tag_expect, m.tag, 16);
+            d.result = idx[j];
+            R += d.rows;
+        }
+        const uint64_t Q = std::max<uint64_t>(1, (R + W - 1) / W);
+        uint32_t w = 0, nch = 0;
+        uint64_t budget = Q;
+        wf[0] = 0;
+        for (size_t j = 0; j < idx.size(); j++) {
+            uint32_t r = 0;
+            while (r < mm[j].rows) {
+                const uint32_t take = (uint32_t)std::min<uint64_t>(budget, mm[j].rows - r);
+                ch[nch].msg = (uint32_t)j; ch[nch].r0 = r; ch[nch].r1 = r + take;
+                nch++; r += take; budget -= take;
+                if (budget == 0) { wf[++w] = nch; budget = Q; }
+            }
+        }
+        if (wf[w] != nch) wf[++w] = nch;
+        const uint32_t n_warps = w;
+
+        MultiParams p;
+        memset(&p, 0, sizeof(p));
+        gcm_ctx *c = groups[k].ctx;
+        memcpy(p.rk, c->h_rk, sizeof(p.rk));
+        p.tab.te0 = c->d_te0; p.tab.ktab = c->d_ktab; p.tab.hpow = c->d_hpow; p.tab.hx = c->d_hx; p.tab.h = c->d_h;
+        p.msgs = (const MultiMsg *)(g.d_multi + lay[k].msgs);
+        p.chunks = (const MultiChunk *)(g.d_multi + lay[k].chunks);
+        p.warp_first = (const uint32_t *)(g.d_multi + lay[k].wfirst);
+        p.n_msgs = (uint32_t)idx.size();
+        p.n_warps = n_warps;
+        p.acc = (unsigned long long *)(g.d_multi + lay[k].acc);
+        p.counter = (unsigned *)(g.d_multi + lay[k].counter);
+        p.results = (MultiResult *)g.d_res;
+        // one upload per group: descriptors, chunks, chunk ranges and the zeroed accumulators / ticket
+        const size_t lo = lay[k].msgs, hi = lay[k].counter + 256;
+        CUB(cudaMemcpyAsync(g.d_multi + lo, g.h_multi + lo, hi - lo, cudaMemcpyHostToDevice, s));
+        const int blocks = (int)((n_warps + MULTI_THREADS / 32 - 1) / (MULTI_THREADS / 32));
+        const MultiMsg *d_msgs = p.msgs;
+        cudaError_t e = launch_multi(c->nr, decrypt ? MODE_DECRYPT : MODE_ENCRYPT, blocks, p, s);
+        secure_zero(&p, sizeof(p));
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+        if (decrypt) {
+            launch_multi_wipe(d_msgs, (const MultiResult *)g.d_res, (uint32_t)idx.size(), s);
+            CUB(cudaGetLastError());
+        }
+    }
+    return GCM_OK;
+}
 
 int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
 {
@@ -419,13 +547,21 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
         if (m.len >= BATCH_LARGE_BYTES) large.push_back(i);
         else small[m.key_bits == 256].push_back(i);
     }
-    // longest first: the tail of the ticket queue is then made of short messages
+    // longest first: the tail of the ticket queue is then made of short messages.  Counting sort on
+    // the row count (32 blocks = 512 bytes per row; small messages have at most BATCH_LARGE_BYTES / 512 rows).
     uint32_t pos = 0, start[2], count[2];
-    for (int k = 0; k < 2; k++) {
-        std::stable_sort(small[k].begin(), small[k].end(),
-                         [&](uint32_t a, uint32_t b) { return msgs[a].len > msgs[b].len; });
-        start[k] = pos; count[k] = (uint32_t)small[k].size();
-        for (uint32_t i : small[k]) g.h_order[pos++] = i;
+    {
+        constexpr uint32_t kBuckets = (uint32_t)(BATCH_LARGE_BYTES / 512) + 2;
+        std::vector<uint32_t> head(kBuckets + 1);
+        for (int k = 0; k < 2; k++) {
+            start[k] = pos; count[k] = (uint32_t)small[k].size();
+            std::fill(head.begin(), head.end(), 0u);
+            auto bucket = [&](uint32_t i) { return kBuckets - 1 - (uint32_t)((msgs[i].len + 511) / 512); };   // descending
+            for (uint32_t i : small[k]) head[bucket(i) + 1]++;
+            for (uint32_t b = 0; b < kBuckets; b++) head[b + 1] += head[b];
+            for (uint32_t i : small[k]) g.h_order[pos + head[bucket(i)]++] = i;
+            pos += count[k];
+        }
     }
     CUB(cudaMemcpyAsync(g.d_desc, g.h_desc, (size_t)n * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
     if (pos) CUB(cudaMemcpyAsync(g.d_order, g.h_order, (size_t)pos * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
@@ -442,23 +578,15 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
                                 : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s);
         if (e != cudaSuccess) return gcm_cuda_fail(e);
     }
-    for (uint32_t i : large) {
-        gcm_msg &m = msgs[i];
-        gcm_ctx *c = nullptr;
-        rc = ctx_for_key_locked(m.key, m.key_bits, s, &c);
-        if (rc == GCM_OK) {
-            rc = decrypt ? gcm_decrypt_verify_async(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out,
-                                                    g.d_desc[i].tag, &g.d_res[i].status, s)
-                         : gcm_encrypt_async(c, m.iv, m.d_aad, m.aad_len, m.d_in, m.len, m.d_out, g.d_res[i].tag, s);
-        }
-        if (rc != GCM_OK) { m.status = rc; if (first_err == GCM_OK) first_err = rc; }
-    }
+    rc = run_large_locked(msgs, large, decrypt, s, &first_err);
+    if (rc != GCM_OK) return rc;
     CUB(cudaMemcpyAsync(g.h_res, g.d_res, (size_t)n * sizeof(BatchResult), cudaMemcpyDeviceToHost, s));
     // the descriptors hold raw keys: wipe the device copy on the stream, the host copy after the sync
     launch_wipe((uint8_t *)g.d_desc, (uint64_t)n * sizeof(BatchDesc), nullptr, s);
     CUB(cudaGetLastError());
     CUB(cudaStreamSynchronize(s));
     secure_zero(g.h_desc, (size_t)n * sizeof(BatchDesc));
+    if (g.by_key.size() > BatchState::kMaxKeys) evict_keys_locked();     // nothing is in flight after the sync
     int failures = 0;
     for (uint32_t i = 0; i < n; i++) {
         gcm_msg &m = msgs[i];

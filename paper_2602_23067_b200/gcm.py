@@ -22,7 +22,9 @@ EXPORTED_SYMBOLS = [
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
     "gcm_encrypt_host", "gcm_decrypt_verify_host",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
+    "gcm_measure_pipe_rates",
 ]
+RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad"]
 
 
 class GcmError(RuntimeError):
@@ -84,6 +86,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_batch_release.argtypes = []
     L.gcm_batch_release.restype = None
+    L.gcm_measure_pipe_rates.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+    L.gcm_measure_pipe_rates.restype = ctypes.c_int
     return L
 
 
@@ -322,6 +326,13 @@ def gcm_decrypt_verify_batch(msgs: Iterable[dict], stream=None) -> List[int]:
 
 def gcm_batch_release() -> None:
     _L.gcm_batch_release()
+
+
+def gcm_measure_pipe_rates() -> dict:
+    """Thread-operations per SM-cycle of the instruction classes in RATE_NAMES, measured on the device."""
+    out = (ctypes.c_double * len(RATE_NAMES))()
+    _check(_L.gcm_measure_pipe_rates(out, len(RATE_NAMES)), "gcm_measure_pipe_rates")
+    return {k: float(out[i]) for i, k in enumerate(RATE_NAMES)}
 
 
 class Context:

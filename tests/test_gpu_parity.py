@@ -422,3 +422,13 @@ def test_host_pipeline_multi_chunk(G, oracle):
         assert not bool(back.any().item())
     finally:
         G.gcm_destroy(ctx)
+
+
+def test_pipe_rate_probe(G):
+    """gcm_measure_pipe_rates: the shared-memory data pipe serves one 128-byte wavefront per SM-cycle
+    (32 four-byte or 8 sixteen-byte lookups), the ALU and FMA pipes 64 lanes each."""
+    r = G.gcm_measure_pipe_rates()
+    assert set(r) == set(G.RATE_NAMES)
+    assert 24 <= r["lds32"] <= 33 and 6 <= r["lds128"] <= 8.3
+    assert 48 <= r["lop3"] <= 66 and 48 <= r["prmt"] <= 66 and 48 <= r["imad"] <= 66
+    assert r["lop3_imad"] > r["lop3"]
