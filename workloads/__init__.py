@@ -213,3 +213,39 @@ def config_c5(payload_bytes: int = 4 << 30, with_payload: bool = True) -> Messag
     flip = int(rng.integers(0, 8 * payload_bytes))
     payload = random_payload(rng, payload_bytes) if with_payload else np.zeros(0, np.uint8)
     return Message(key, iv, aad, payload, "C5", {"flip_bit": flip, "payload_bytes": payload_bytes})
+
+
+# -------------------------------------------------------------------------------------------------
+# Whole FITS files for the authenticated-container path (section 3.2.2; the
+# validation file of L245 is a 256 x 256 float32 image "with representative WCS metadata").
+# -------------------------------------------------------------------------------------------------
+@dataclass
+class FitsFrame:
+    fits: bytes          # a single-HDU FITS file: header block(s) + big-endian float32 data unit
+    key_h: bytes         # Header Key
+    key_d: bytes         # Data Key
+    nonce_h: bytes       # 96-bit nonces (the paper draws them from the OS entropy pool, L137;
+    nonce_d: bytes       # here they are seeded so that both implementations build the same bytes)
+    ny: int = 0
+    nx: int = 0
+
+
+def fits_frame(seed: int = 2001, ny: int = 256, nx: int = 256, key_bytes: int = 16,
+               n_sources: int = 20, extra_cards: int = 0) -> FitsFrame:
+    """Draw order: key_h -> key_d -> nonce_h -> nonce_d -> header -> pixels.  extra_cards > 0 appends
+    HISTORY cards so that the header spans several 2880-byte blocks."""
+    rng = _rng(seed)
+    key_h = _bytes(rng, key_bytes).tobytes()
+    key_d = _bytes(rng, key_bytes).tobytes()
+    nonce_h = _bytes(rng, 12).tobytes()
+    nonce_d = _bytes(rng, 12).tobytes()
+    hdr = fits_header_block(rng, nx, ny).tobytes()
+    if extra_cards:
+        text = hdr.decode("ascii")
+        end = text.index("END".ljust(80))
+        body = text[:end] + "".join(("HISTORY synthetic processing step %05d" % i).ljust(80) for i in range(extra_cards))
+        body += "END".ljust(80)
+        body += " " * ((-len(body)) % FITS_BLOCK)
+        hdr = body.encode("ascii")
+    data = fits_image_payload(rng, ny, nx, n_sources=n_sources).tobytes()
+    return FitsFrame(hdr + data, key_h, key_d, nonce_h, nonce_d, ny, nx)
