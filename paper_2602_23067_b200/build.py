@@ -8,7 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libb200gcm.so")
-SOURCES = ["gcm_api.cu", "gcm_setup.cu", "gcm_fused.cu", "gcm_batch.cu", "gcm_multi.cu", "gcm_host.cu", "gcm_rates.cu"]
+SOURCES = ["gcm_api.cu", "gcm_setup.cu", "gcm_fused.cu", "gcm_batch.cu", "gcm_multi.cu", "gcm_host.cu", "gcm_rates.cu",
+           "fits_sum.cu", "gfc_frame.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
@@ -19,7 +20,7 @@ NVCC_FLAGS = [
 
 def _newest_source_mtime() -> float:
     paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    paths.append(os.path.join(os.path.dirname(HERE), "include", "gcm.h"))
+    paths += [os.path.join(os.path.dirname(HERE), "include", f) for f in ("gcm.h", "gfc.h")]
     return max(os.path.getmtime(p) for p in paths)
 
 

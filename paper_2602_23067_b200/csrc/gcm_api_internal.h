@@ -36,3 +36,7 @@ struct GcmParams;
 int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
                      const void *d_in, uint64_t len, void *d_out, uint32_t ctr_base, GcmParams *p, int *blocks);
 void gcm_host_pipe_free(gcm_ctx *c);
+// gcm_host.cu: the chunked host-buffer pipeline behind gcm_encrypt_host / gcm_decrypt_verify_host.
+int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
+                 const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream,
+                 unsigned long long *d_sum32);

@@ -18,6 +18,7 @@
 #include "gcm_setup.cuh"
 #include "gcm_fused.cuh"
 #include "gcm_api_internal.h"
+#include "fits_sum.cuh"
 
 #define PIPE_SLOTS 3
 #define PIPE_CHUNK_BYTES (64ull << 20)   /* multiple of 16 */
@@ -104,8 +105,11 @@ void gcm_host_pipe_free(gcm_ctx *c)
     c->pipe = nullptr;
 }
 
-static int run_host(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
-                    const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream)
+// d_sum32 (device, may be NULL): every chunk's ciphertext is also added to the FITS DATASUM accumulator
+// while it is still in the staging buffer (the container layer of gfc_frame.cu).
+int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
+                 const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream,
+                 unsigned long long *d_sum32)
 {
     if (!c || !iv || !tag_io) return GCM_ERR_ARG;
     if (len > ((1ull << 36) - 32) || aad_len >= (1ull << 32)) return GCM_ERR_LEN;
@@ -157,6 +161,7 @@ static int run_host(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, 
         memset(&p, 0, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
         CU(cudaEventRecord(hp->kernel_done[slot], s));
+        if (d_sum32 && mode == MODE_ENCRYPT) CU(launch_fits_sum32(hp->d_stage[slot], clen, d_sum32, c->sm_count, s));
         if (clen) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
         if (last) {
             if (mode == MODE_ENCRYPT) CU(cudaMemcpyAsync(c->h_pinned, c->d_tag, 16, cudaMemcpyDeviceToHost, s));
@@ -180,7 +185,7 @@ static int run_host(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, 
 extern "C" int gcm_encrypt_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
                                 const void *h_pt, uint64_t len, void *h_ct, uint8_t tag[16], void *stream)
 {
-    return run_host(c, MODE_ENCRYPT, iv, h_aad, aad_len, h_pt, len, h_ct, tag, stream);
+    return gcm_host_run(c, MODE_ENCRYPT, iv, h_aad, aad_len, h_pt, len, h_ct, tag, stream, nullptr);
 }
 
 extern "C" int gcm_decrypt_verify_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
@@ -188,5 +193,5 @@ extern "C" int gcm_decrypt_verify_host(gcm_ctx *c, const uint8_t iv[12], const v
 {
     uint8_t t[16];
     memcpy(t, tag, 16);
-    return run_host(c, MODE_DECRYPT, iv, h_aad, aad_len, h_ct, len, h_pt, t, stream);
+    return gcm_host_run(c, MODE_DECRYPT, iv, h_aad, aad_len, h_ct, len, h_pt, t, stream, nullptr);
 }

@@ -14,9 +14,9 @@ def lib_path():
     return build.build()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "gcm.h")).read()
-    return sorted(set(re.findall(r"GCM_API\s+[\w \*]+?\b(gcm_\w+)\s*\(", text)))
+def declared_symbols(header="gcm.h", prefix="gcm_"):
+    text = open(os.path.join(ROOT, "include", header)).read()
+    return sorted(set(re.findall(r"GCM_API\s+[\w \*]+?\b(%s\w+)\s*\(" % prefix, text)))
 
 
 def test_header_declares_the_boundary():
@@ -28,7 +28,7 @@ def test_header_declares_the_boundary():
 
 def test_library_exports_every_declared_symbol(lib_path):
     L = ctypes.CDLL(lib_path)
-    for name in declared_symbols():
+    for name in declared_symbols() + declared_symbols("gfc.h", "gfc_"):
         assert hasattr(L, name), name
     L.gcm_version.restype = ctypes.c_char_p
     assert b"sm_100a" in L.gcm_version()
@@ -38,6 +38,9 @@ def test_binding_lists_the_same_symbols(lib_path):
     import paper_2602_23067_b200 as pkg
     assert sorted(pkg.EXPORTED_SYMBOLS) == declared_symbols()
     assert pkg.library_path() == lib_path
+    from paper_2602_23067_b200 import gfc
+    assert sorted(gfc.EXPORTED_SYMBOLS) == declared_symbols("gfc.h", "gfc_")
+    assert len(gfc.EXPORTED_SYMBOLS) == 5
 
 
 def test_argument_errors_without_gpu(lib_path):
@@ -49,6 +52,8 @@ def test_argument_errors_without_gpu(lib_path):
     L = ctypes.CDLL(lib_path)
     assert L.gcm_init(None, b"0" * 16, 128) == pkg.GCM_ERR_ARG
     assert L.gcm_encrypt(None, None, None, 0, None, 0, None, None, None) == pkg.GCM_ERR_ARG
+    assert L.gfc_context_create(None, 0, 0) == pkg.GCM_ERR_ARG
+    assert L.gfc_encrypt_frame(None, None, 0, None, None, 128, None, None, None) == pkg.GCM_ERR_ARG
 
 
 def test_no_cpu_fallback_in_product_path():
