@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-mib", type=float, default=384.0)
     ap.add_argument("--workload", default="c5",
-                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency"],
+                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum"],
                     help="c5 = the headline (default); the others are the supplementary measurements of DESIGN.md section 10")
     return ap.parse_args()
 
@@ -479,6 +479,60 @@ def run_extra(args):
                               "note": "peak is the large-message bound of the 8-bit-table kernel; the per-message key schedule, "
                                       "H ladder and 4-bit table build of this kernel are not in it"},
                     ms_per_step_median=statistics.median(per))
+    elif w == "datasum":
+        # DATASUM reduction kernel (FITS checksum of the encrypted payload): HBM-bound, 1 byte read per byte
+        from paper_2602_23067_b200 import gfc
+        n = int(args.size_mib * (1 << 20))
+        data = rand_bytes(n, 31)
+        acc = torch.zeros(1, dtype=torch.int64, device="cuda")
+        total_ms, per, clocks = timed(lambda: gfc.gfc_datasum_async(data, acc, stream))
+        gbs = steps * n / (total_ms * 1e-3) / 1e9
+        hbm = float(peaks["hbm_gbs"])
+        line.update(metric="FITS DATASUM kernel GB/s (device-timed, %d MiB)" % (n >> 20), value=gbs, ms_per_step=total_ms / steps,
+                    config={"workload": "datasum: 1's-complement sum of big-endian 32-bit words over a %d-byte device buffer "
+                                        "(larger than L2; no flush needed)" % n, "payload_bytes": n},
+                    gpu_launches=steps, clocks=clocks,
+                    roofline={"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": UNIT, "frac": gbs / hbm,
+                              "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["_source"], "traffic": None,
+                              "algorithmic_bytes_per_launch": n},
+                    ms_per_step_median=statistics.median(per))
+    elif w == "frame":
+        # The authenticated FITS container end to end (include/gfc.h; PAPER.md sections 3.2.2, 3.3.2, 4.2): host buffers in,
+        # host buffers out, header message on streamH concurrently with the chunked data pipeline on streamD.
+        from paper_2602_23067_b200 import gfc
+        out = {}
+        for name, ny, nx in (("256x256", 256, 256), ("4096x4096", 4096, 4096)):
+            f = workloads.fits_frame(seed=2100, ny=ny, nx=nx, key_bytes=32, n_sources=50)
+            h_fits = torch.frombuffer(bytearray(f.fits), dtype=torch.uint8).pin_memory()
+            ctx = gfc.gfc_context_create(16 * 2880, len(f.fits))
+            r = gfc.gfc_encrypt_frame(ctx, h_fits, f.key_h, f.key_d, f.nonce_h, f.nonce_d)
+            h_cont = torch.from_numpy(r.view().copy()).pin_memory()
+            res = {}
+            for what, call in (("encrypt", lambda: gfc.gfc_encrypt_frame(ctx, h_fits, f.key_h, f.key_d, f.nonce_h, f.nonce_d)),
+                               ("decrypt", lambda: gfc.gfc_decrypt_frame(ctx, h_cont, f.key_h, f.key_d)),
+                               ("decrypt_header_only", lambda: gfc.gfc_decrypt_frame(ctx, h_cont, f.key_h, None))):
+                for _ in range(warm):
+                    call()
+                ts, hm, dm = [], [], []
+                for _ in range(max(steps, 10)):
+                    t0 = time.perf_counter()
+                    r = call()
+                    ts.append(time.perf_counter() - t0)
+                    hm.append(r.header_ms); dm.append(r.data_ms)
+                med = statistics.median(ts)
+                res[what] = {"wall_ms_median": med * 1e3, "file_GBps": len(f.fits) / med / 1e9,
+                             "header_stream_ms": statistics.median(hm), "data_stream_ms": statistics.median(dm),
+                             "warning_code": r.warning_code}
+            full = gfc.gfc_decrypt_frame(ctx, h_cont, f.key_h, f.key_d)
+            assert full.warning_code == 0 and bytes(full.view()[:5760]) == f.fits[:5760]
+            gfc.gfc_context_destroy(ctx)
+            out[name] = dict(res, file_bytes=len(f.fits))
+        big = out["4096x4096"]
+        line.update(metric="authenticated FITS container: gfc_decrypt_frame of a 64 MiB image, file GB/s end to end (host wall clock)",
+                    value=big["decrypt"]["file_GBps"], ms_per_step=big["decrypt"]["wall_ms_median"],
+                    gpu_launches=None, frames=out,
+                    config={"workload": "frame: gfc_encrypt_frame / gfc_decrypt_frame (AES-256, dual key) on a 256x256 and a 4096x4096 float32 "
+                                        "FITS file in pinned host memory; H2D and D2H inside the timed region (PCIe-bound)"})
     elif w == "latency":
         # single-message latency through the synchronous non-batched call (C4's report): host wall clock
         m = workloads.config_c1(payload_bytes=0)

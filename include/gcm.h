@@ -161,7 +161,7 @@ GCM_API int gcm_decrypt_verify_async(gcm_ctx *ctx, const uint8_t iv[12],
  * Host-buffer forms (the paper's data plane stages files through pinned host memory and overlaps
  * the transfers with the kernels on CUDA streams): `h_*` are HOST
  * pointers (pinned memory gives full PCIe rate; pageable memory works).  The message is cut into
- * 64 MiB chunks that travel H2D -> fused kernel -> D2H on three internal streams; the running
+ * chunks (about eight per message, 4 MiB to 64 MiB each) that travel H2D -> fused kernel -> D2H on three internal streams; the running
  * GHASH state is handed from chunk to chunk on the device.  Work already queued on `cuda_stream`
  * is waited for; the call returns when the output and the tag / verdict are in host memory.
  * On GCM_ERR_AUTH h_pt[0..len) is zero-filled.  aad_len < 2^32 here.

@@ -104,6 +104,14 @@ GCM_API int gfc_decrypt_frame(gfc_context *ctx, const uint8_t *container, uint64
  */
 GCM_API int gfc_datasum(const void *d_data, uint64_t len, uint32_t *sum, void *cuda_stream);
 
+/*
+ * Asynchronous form for device-timed measurement and for summing a data unit piece by piece: adds the
+ * sum of d_data[0, len) to *d_acc (device, one uint64 the caller zeroes first; pieces must start at
+ * multiples of 4 bytes of the data unit).  No synchronisation.  The DATASUM is the accumulator folded
+ * with end-around carry: s = (s & 0xFFFFFFFF) + (s >> 32) until s < 2^32.
+ */
+GCM_API int gfc_datasum_async(const void *d_data, uint64_t len, void *d_acc, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,7 +21,8 @@
 #include "fits_sum.cuh"
 
 #define PIPE_SLOTS 3
-#define PIPE_CHUNK_BYTES (64ull << 20)   /* multiple of 16 */
+#define PIPE_CHUNK_BYTES (64ull << 20)   /* staging buffer = largest chunk; multiple of 16 */
+#define PIPE_MIN_CHUNK_BYTES (4ull << 20)
 
 struct HostPipe {
     cudaStream_t stream[PIPE_SLOTS];
@@ -120,7 +121,11 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
     HostPipe *hp = c->pipe;
     cudaStream_t us = (cudaStream_t)user_stream;
 
-    const uint64_t chunk = PIPE_CHUNK_BYTES;
+    // about eight chunks per message so that H2D, kernel and D2H of neighbouring chunks overlap also for
+    // FITS-sized (tens of MiB) messages; 4 MiB at least (launch and table-fill cost), 64 MiB at most (staging)
+    uint64_t chunk = ((len / 8 + (1ull << 20) - 1) >> 20) << 20;
+    if (chunk < PIPE_MIN_CHUNK_BYTES) chunk = PIPE_MIN_CHUNK_BYTES;
+    if (chunk > PIPE_CHUNK_BYTES) chunk = PIPE_CHUNK_BYTES;
     const uint64_t n_chunks = len ? (len + chunk - 1) / chunk : 1;
     const uint64_t last_len = len - (n_chunks - 1) * chunk;
     // work already queued on the caller's stream happens before ours

@@ -17,7 +17,8 @@ from .gcm import GCM_OK, GcmError
 GFC_ERR_FORMAT, GFC_ERR_CAPACITY = -5, -6
 GFC_FULL_ACCESS, GFC_HEADER_FALLBACK, GFC_PAYLOAD_SUPPRESSED = 0, 1, 2
 
-EXPORTED_SYMBOLS = ["gfc_context_create", "gfc_context_destroy", "gfc_encrypt_frame", "gfc_decrypt_frame", "gfc_datasum"]
+EXPORTED_SYMBOLS = ["gfc_context_create", "gfc_context_destroy", "gfc_encrypt_frame", "gfc_decrypt_frame", "gfc_datasum",
+                    "gfc_datasum_async"]
 
 
 class FitsOperationResult(ctypes.Structure):
@@ -42,6 +43,7 @@ _L.gfc_encrypt_frame.argtypes = [_vp, _vp, _u64, ctypes.c_char_p, ctypes.c_char_
                                  ctypes.POINTER(FitsOperationResult)]
 _L.gfc_decrypt_frame.argtypes = [_vp, _vp, _u64, ctypes.c_char_p, ctypes.c_char_p, _ci, ctypes.POINTER(FitsOperationResult)]
 _L.gfc_datasum.argtypes = [_vp, _u64, ctypes.POINTER(ctypes.c_uint32), _vp]
+_L.gfc_datasum_async.argtypes = [_vp, _u64, _vp, _vp]
 
 
 class FrameError(GcmError):
@@ -130,3 +132,10 @@ def gfc_datasum(d_data, stream=None) -> int:
     out = ctypes.c_uint32(0)
     _gcm._check(_L.gfc_datasum(ptr, n, ctypes.byref(out), _gcm._stream(stream)), "gfc_datasum")
     return int(out.value)
+
+
+def gfc_datasum_async(d_data, d_acc, stream=None) -> None:
+    """d_acc: device tensor holding one uint64 (8 bytes), zeroed by the caller; no synchronisation."""
+    ptr, n = _gcm._dev(d_data)
+    acc, _ = _gcm._dev(d_acc)
+    _gcm._check(_L.gfc_datasum_async(ptr, n, acc, _gcm._stream(stream)), "gfc_datasum_async")
