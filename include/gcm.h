@@ -80,8 +80,8 @@ GCM_API int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits);
 GCM_API void gcm_destroy(gcm_ctx *ctx);
 
 /*
- * Launch geometry of the fused kernel: `grid` CTAs (0 = one per SM) of `threads` threads (256 or
- * 512; 0 = default 512).  The stride power H^(grid*threads) and its table are rebuilt.  Results
+ * Launch geometry of the fused kernel: `grid` CTAs (0 = one per SM) of `threads` threads (256, 384
+ * or 512; 0 = default 512).  The stride power H^(grid*threads) and its table are rebuilt.  Results
  * never depend on the geometry (geometry-agnostic counters; reading S11).
  * Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
  */

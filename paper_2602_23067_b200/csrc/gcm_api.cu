@@ -107,7 +107,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
 
     int rc = GCM_OK;
     do {
-        if ((e = cudaHostAlloc((void **)&c->h_pinned, 64, cudaHostAllocDefault)) != cudaSuccess) break;
+        if ((e = cudaHostAlloc((void **)&c->h_pinned, 64, cudaHostAllocMapped)) != cudaSuccess) break;
         if ((e = cudaMemset(c->d_slab, 0, c->slab_bytes)) != cudaSuccess) break;
         SetupParams sp = setup_params(c, key);
         launch_setup(sp, 0);
@@ -148,7 +148,7 @@ extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)
     if (!c) return GCM_ERR_ARG;
     if (grid == 0) grid = c->sm_count;
     if (threads == 0) threads = GCM_MAX_THREADS;
-    if (grid < 1 || grid > GCM_MAX_GRID || (threads != 256 && threads != 512)) return GCM_ERR_ARG;
+    if (grid < 1 || grid > GCM_MAX_GRID || (threads != 256 && threads != 384 && threads != 512)) return GCM_ERR_ARG;
     // no table depends on the geometry: the GHASH stride power is H^32 for every launch shape
     c->grid = grid;
     c->threads = threads;
@@ -292,9 +292,10 @@ extern "C" int gcm_encrypt(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, 
                            const void *d_pt, uint64_t len, void *d_ct, uint8_t tag[16], void *stream)
 {
     if (!c || !tag) return GCM_ERR_ARG;
-    int rc = gcm_encrypt_async(c, iv, d_aad, aad_len, d_pt, len, d_ct, c->d_tag, stream);
+    // the finishing thread stores the tag straight into mapped pinned host memory (unified addressing):
+    // one posted PCIe write instead of a separate D2H copy on the latency path
+    int rc = gcm_encrypt_async(c, iv, d_aad, aad_len, d_pt, len, d_ct, c->h_pinned, stream);
     if (rc != GCM_OK) return rc;
-    CU(cudaMemcpyAsync(c->h_pinned, c->d_tag, 16, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     memcpy(tag, c->h_pinned, 16);
     return GCM_OK;
@@ -309,11 +310,11 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
     int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, &p, &blocks);
     if (rc != GCM_OK) return rc;
     memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
+    p.status = (int *)(c->h_pinned + 16);   // verdict written straight into mapped pinned host memory
     CU(cudaSetDevice(c->device));
     cudaError_t e = launch_fused(c->nr, MODE_DECRYPT, c->threads, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
-    CU(cudaMemcpyAsync(c->h_pinned + 16, c->d_status, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     int status;
     memcpy(&status, c->h_pinned + 16, 4);

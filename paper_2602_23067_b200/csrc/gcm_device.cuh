@@ -185,7 +185,10 @@ __device__ __forceinline__ void st16_stream(uint8_t *p, uint4 v)
 static __device__ __noinline__ uint4 load_bytes(const uint8_t *p, uint32_t n)
 {
     uint32_t w[4] = {0, 0, 0, 0};
-    for (uint32_t i = 0; i < n; i++) w[i >> 2] |= (uint32_t)p[i] << (8 * (i & 3));
+    uint32_t i = 0;
+    if ((reinterpret_cast<uintptr_t>(p) & 3) == 0)          // whole words first when the pointer allows it
+        for (; i + 4 <= n; i += 4) w[i >> 2] = *reinterpret_cast<const uint32_t *>(p + i);
+    for (; i < n; i++) w[i >> 2] |= (uint32_t)p[i] << (8 * (i & 3));
     return make_uint4(w[0], w[1], w[2], w[3]);
 }
 static __device__ __noinline__ void store_bytes(uint8_t *p, uint4 v, uint32_t n)
@@ -229,16 +232,53 @@ __device__ __forceinline__ uint4 cta_xor_reduce(uint4 v, uint4 *red)
     return v;
 }
 
+// Table fill at kernel start, latency-critical for small messages (header-sized messages): all
+// global loads of a thread are issued before its first shared-memory store, so the fill costs about one L2
+// round trip plus the 1536 store wavefronts of the 192 KB, instead of one round trip per loop iteration.
 template <int TPB>
 __device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const uint32_t *te0)
 {
     uint32_t *a0 = reinterpret_cast<uint32_t *>(sm + AES_A0_OFF);
     uint32_t *a1 = reinterpret_cast<uint32_t *>(sm + AES_A1_OFF);
-    for (uint32_t j = threadIdx.x; j < 16384; j += TPB) {
-        uint32_t te = __ldg(te0 + (j >> 6));
-        bool odd = (j >> 5) & 1;
-        a0[j] = odd ? rotl32(te, 8) : te;            // T0 | T1
-        a1[j] = odd ? rotl32(te, 24) : rotl32(te, 16); // T2 | T3
+    constexpr int ROWS = (256 * 64 + TPB - 1) / TPB;       // table words per thread and array
+    uint32_t te[ROWS];
+#pragma unroll
+    for (int k = 0; k < ROWS; k++) {
+        const uint32_t j = threadIdx.x + k * TPB;
+        te[k] = j < 16384 ? __ldg(te0 + (j >> 6)) : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < ROWS; k++) {
+        const uint32_t j = threadIdx.x + k * TPB;
+        if (j < 16384) {
+            const bool odd = (j >> 5) & 1;
+            a0[j] = odd ? rotl32(te[k], 8) : te[k];                 // T0 | T1
+            a1[j] = odd ? rotl32(te[k], 24) : rotl32(te[k], 16);    // T2 | T3
+        }
     }
 }
 
+// The GHASH multiplier table: global loads into registers first (ktab_load), stores after the AES tables
+// have been written (ktab_store), so the two fills share one memory round trip.
+template <int TPB>
+struct KtabRegs { uint4 v[(KTAB_BYTES / 16 + TPB - 1) / TPB]; };
+
+template <int TPB>
+__device__ __forceinline__ void ktab_load(KtabRegs<TPB> &r, const uint4 *ktab)
+{
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(r.v) / sizeof(uint4)); k++) {
+        const uint32_t j = threadIdx.x + k * TPB;
+        r.v[k] = j < KTAB_BYTES / 16 ? __ldg(ktab + j) : make_uint4(0, 0, 0, 0);
+    }
+}
+template <int TPB>
+__device__ __forceinline__ void ktab_store(const KtabRegs<TPB> &r, uint8_t *sm)
+{
+    uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(r.v) / sizeof(uint4)); k++) {
+        const uint32_t j = threadIdx.x + k * TPB;
+        if (j < KTAB_BYTES / 16) kt[j] = r.v[k];
+    }
+}

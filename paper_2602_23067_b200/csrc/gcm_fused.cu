@@ -32,20 +32,31 @@
 
 // H^d for d < 2^36 from the radix-512 digit table: four factors, two multiply levels, every lane
 // of the warp takes part (lane & 3 picks the digit) and ends up with the product.
-__device__ __forceinline__ uint4 warp_h_power(const uint4 *hx, uint64_t d, uint32_t lane)
+__device__ __forceinline__ uint4 warp_h_power(const uint4 *hx, uint64_t d, uint32_t lane, uint64_t d_max)
 {
     const uint32_t k = lane & 3;
     const uint32_t digit = (uint32_t)(d >> (HX_RADIX_BITS * k)) & ((1u << HX_RADIX_BITS) - 1);
     uint4 f = __ldg(hx + (k << HX_RADIX_BITS) + digit);
-#pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
+    // d_max (launch-uniform bound on d) says how many digits can be non-zero: short messages skip levels
+    const int levels = d_max < (1ull << HX_RADIX_BITS) ? 0 : (d_max < (1ull << (2 * HX_RADIX_BITS)) ? 1 : 2);
+    for (int o = 1; o <= levels; o++) {
+        const int m = 1 << (o - 1);
         uint4 g;
-        g.x = __shfl_xor_sync(0xFFFFFFFFu, f.x, o); g.y = __shfl_xor_sync(0xFFFFFFFFu, f.y, o);
-        g.z = __shfl_xor_sync(0xFFFFFFFFu, f.z, o); g.w = __shfl_xor_sync(0xFFFFFFFFu, f.w, o);
+        g.x = __shfl_xor_sync(0xFFFFFFFFu, f.x, m); g.y = __shfl_xor_sync(0xFFFFFFFFu, f.y, m);
+        g.z = __shfl_xor_sync(0xFFFFFFFFu, f.z, m); g.w = __shfl_xor_sync(0xFFFFFFFFu, f.w, m);
         f = gf_mul_mem(f, g);
     }
+    // lanes with k = 0 hold the product of the digits that can be non-zero; hand it to every lane
+    f.x = __shfl_sync(0xFFFFFFFFu, f.x, lane & ~3u); f.y = __shfl_sync(0xFFFFFFFFu, f.y, lane & ~3u);
+    f.z = __shfl_sync(0xFFFFFFFFu, f.z, lane & ~3u); f.w = __shfl_sync(0xFFFFFFFFu, f.w, lane & ~3u);
     return f;
 }
+
+#ifdef GCM_PHASE_PROBE      // _work latency probe only: clock64 stamps of CTA 0 / thread 0 behind the partials
+#define STAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) ((long long *)(p.partials + 4000))[i] = clock64(); } while (0)
+#else
+#define STAMP(i) do { } while (0)
+#endif
 
 template <int NR, int MODE, int TPB>
 __global__ void __launch_bounds__(TPB, 1)
@@ -53,6 +64,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
 {
     extern __shared__ __align__(1024) uint8_t sm[];
     __shared__ bool s_last;
+    __shared__ uint4 s_ekj0;
     const uint32_t t = threadIdx.x, lane = t & 31, lane4 = lane * 4;
     // broadcast from lane 0: tells the compiler the warp index (and the row loop below) is warp-uniform,
     // so the shared-memory base stays in a uniform register and folds into every LDS address
@@ -66,24 +78,36 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     const uint32_t r0 = r0_64 < S ? (uint32_t)r0_64 : S;
     const uint32_t r1 = (uint64_t)r0 + Q < S ? r0 + Q : S;
     const bool has_rows = r0 < r1;
+    STAMP(0);
 
-    if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
     {
-        uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
-        for (uint32_t j = t; j < KTAB_BYTES / 16; j += TPB) kt[j] = __ldg(p.tab.ktab + j);
+        KtabRegs<TPB> kr;
+        ktab_load<TPB>(kr, p.tab.ktab);
+        if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
+        ktab_store<TPB>(kr, sm);
     }
     // position weight of the warp's run, H^(blocks behind it): computed while the tables arrive
     uint4 wpow = make_uint4(0, 0, 0, 0);
     const bool tail_warp = has_rows && r1 == S;          // owns the last (possibly ragged) row
-    if (has_rows && !tail_warp) wpow = warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane);
+    if (has_rows && !tail_warp) wpow = warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane, p.vblocks);
     __syncthreads();
+    STAMP(1);
 
     uint32_t sel[8];
 #pragma unroll
     for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
     CtrConst cc = {0, 0, 0, 0};
     CtrCache cu = {0, 0, 0, 0};
-    if (MODE != MODE_GHASH) cc = ctr_const(p.rk, p.iv[0], p.iv[1], p.iv[2], sm, lane4);
+    if (MODE != MODE_GHASH) {
+        cc = ctr_const(p.rk, p.iv[0], p.iv[1], p.iv[2], sm, lane4);
+        // a3: E_K(J0), J0 = IV || 0^31 || 1, by the last warp of every CTA while the others start their rows
+        // (any CTA may turn out to be the finisher); it reaches the finishing thread through shared memory
+        if (warp == TPB / 32 - 1) {
+            const CtrCache c1 = ctr_cache(p.rk, sm, lane4, cc, 1u);
+            const uint4 ek = aes_ctr_block<NR>(p.rk, sm, lane4, cc, c1, 1u);
+            if (lane == 0) s_ekj0 = ek;
+        }
+    }
 
     uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
@@ -135,6 +159,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         if (fast || valid) Y = xor4(ym, X);
     }
 
+    STAMP(2);
     // a8: lane correction H^(blocks from the lane's last block to the end of the warp's run), XOR over
     // the warp, warp correction H^(blocks behind the run), XOR over the CTA.  In the ragged last row
     // only lanes < rem folded a block; rotating the lane order by rem keeps the exponents in 1..32.
@@ -160,6 +185,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
         }
     }
+    STAMP(3);
     // a9: last-CTA-done combination of the partials
     if (t == 0) {
         p.partials[blockIdx.x] = part;
@@ -169,6 +195,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     }
     __syncthreads();
     if (!s_last) return;
+    STAMP(4);
     __threadfence();
     uint4 acc = make_uint4(0, 0, 0, 0);
     for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
@@ -188,10 +215,8 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         if (MODE == MODE_GHASH) {
             *p.tag_out = Sg;
         } else {
-            // a3 + a11: E_K(J0), J0 = IV || 0^31 || 1; tag; constant-time compare
-            cu = ctr_cache(p.rk, sm, lane4, cc, 1u);
-            const uint4 ek = aes_ctr_block<NR>(p.rk, sm, lane4, cc, cu, 1u);
-            const uint4 tag = xor4(Sg, ek);
+            // a11: tag = E_K(J0) xor S; constant-time compare
+            const uint4 tag = xor4(Sg, s_ekj0);
             if (MODE == MODE_ENCRYPT) {
                 *p.tag_out = tag;
             } else {
@@ -202,6 +227,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             }
         }
         *p.counter = 0;   // ready for the next launch on this context
+        STAMP(5);
     }
 }
 
@@ -236,5 +262,6 @@ static cudaError_t launch_tpb(int nr, int mode, int blocks, const GcmParams &p, 
 cudaError_t launch_fused(int nr, int mode, int threads, int blocks, const GcmParams &p, cudaStream_t s)
 {
     if (threads == 256) return launch_tpb<256>(nr, mode, blocks, p, s);
+    if (threads == 384) return launch_tpb<384>(nr, mode, blocks, p, s);
     return launch_tpb<512>(nr, mode, blocks, p, s);
 }

@@ -40,10 +40,11 @@ gcm_multi_kernel(const __grid_constant__ MultiParams p)
     const uint32_t warp = __shfl_sync(0xFFFFFFFFu, t >> 5, 0);
     const uint32_t wg = blockIdx.x * (MULTI_THREADS / 32) + warp;
 
-    fill_aes_tables<MULTI_THREADS>(sm, p.tab.te0);
     {
-        uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
-        for (uint32_t j = t; j < KTAB_BYTES / 16; j += MULTI_THREADS) kt[j] = __ldg(p.tab.ktab + j);
+        KtabRegs<MULTI_THREADS> kr;
+        ktab_load<MULTI_THREADS>(kr, p.tab.ktab);
+        fill_aes_tables<MULTI_THREADS>(sm, p.tab.te0);
+        ktab_store<MULTI_THREADS>(kr, sm);
     }
     __syncthreads();
 
