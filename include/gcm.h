@@ -212,7 +212,8 @@ typedef struct {
 GCM_API int gcm_encrypt_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
 GCM_API int gcm_decrypt_verify_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
 
-/* Frees the batch path's cached per-key contexts and staging buffers (zeroising key material). */
+/* Frees the batch path's cached per-key contexts and staging buffers (zeroising key material) and the
+ * wiped allocations that gcm_destroy keeps for the next gcm_init. */
 GCM_API void gcm_batch_release(void);
 
 #ifdef __cplusplus

@@ -5,7 +5,9 @@
 #include <stdint.h>
 #include <string.h>
 #include <stdlib.h>
+#include <mutex>
 #include <new>
+#include <vector>
 
 #include "../../include/gcm.h"
 #include "gcm_common.cuh"
@@ -15,6 +17,43 @@
 
 static int g_device = 0;
 static int g_last_cuda_error = 0;
+
+// Wiped (device slab, pinned block) pairs of destroyed contexts, kept for the next gcm_init on the same
+// device: cudaMalloc + cudaHostAlloc cost milliseconds, the setup kernel 56 us (the paper pre-allocates
+// once per session for the same reason).  At most kPoolMax pairs are kept.
+namespace {
+struct PooledSlab { int device; uint8_t *d_slab; size_t bytes; };
+constexpr size_t kPoolMax = 4;
+std::mutex g_pool_mu;
+std::vector<PooledSlab> g_pool;
+
+// 64-byte blocks of mapped pinned memory (tag / verdict of the synchronous calls) come out of one page that
+// is allocated once per process: a cudaHostAlloc per context costs about two milliseconds.
+uint8_t *g_pin_page = nullptr;
+uint64_t g_pin_used = 0;
+
+uint8_t *pin_take()
+{
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (!g_pin_page && cudaHostAlloc((void **)&g_pin_page, 64 * 64, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) {
+        g_pin_page = nullptr;
+        cudaGetLastError();
+    }
+    if (g_pin_page)
+        for (int i = 0; i < 64; i++)
+            if (!(g_pin_used >> i & 1)) { g_pin_used |= 1ull << i; return g_pin_page + 64 * i; }
+    uint8_t *p = nullptr;                                  // page exhausted (more than 64 live contexts)
+    if (cudaHostAlloc((void **)&p, 64, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+
+void pin_give(uint8_t *p)
+{
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (g_pin_page && p >= g_pin_page && p < g_pin_page + 64 * 64) g_pin_used &= ~(1ull << ((p - g_pin_page) / 64));
+    else cudaFreeHost(p);
+}
+}
 
 int gcm_cuda_fail(cudaError_t e)
 {
@@ -70,9 +109,11 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     if (!out || !key || (key_bits != 128 && key_bits != 256)) return GCM_ERR_ARG;
     *out = nullptr;
     CU(cudaSetDevice(g_device));
-    cudaDeviceProp prop;
-    CU(cudaGetDeviceProperties(&prop, g_device));
-    if ((size_t)prop.sharedMemPerBlockOptin < (size_t)FUSED_SMEM_BYTES) return GCM_ERR_CUDA;
+    // two attribute queries, not cudaGetDeviceProperties (which takes milliseconds)
+    int sm_count = 0, smem_optin = 0;
+    CU(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, g_device));
+    CU(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, g_device));
+    if ((size_t)smem_optin < (size_t)FUSED_SMEM_BYTES) return GCM_ERR_CUDA;
 
     gcm_ctx *c = new (std::nothrow) gcm_ctx;
     if (!c) return GCM_ERR_NOMEM;
@@ -80,7 +121,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     c->device = g_device;
     c->key_bits = key_bits;
     c->nr = key_bits == 128 ? 10 : 14;
-    c->sm_count = prop.multiProcessorCount;
+    c->sm_count = sm_count;
     c->grid = c->sm_count;
     c->threads = GCM_MAX_THREADS;
 
@@ -92,7 +133,17 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
     size_t o_cnt = take(4), o_tag = take(16), o_status = take(4);
     c->slab_bytes = off;
-    cudaError_t e = cudaMalloc((void **)&c->d_slab, c->slab_bytes);
+    cudaError_t e = cudaSuccess;
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mu);
+        for (size_t i = 0; i < g_pool.size(); i++)
+            if (g_pool[i].device == g_device && g_pool[i].bytes == c->slab_bytes) {
+                c->d_slab = g_pool[i].d_slab;
+                g_pool.erase(g_pool.begin() + i);
+                break;
+            }
+    }
+    if (!c->d_slab) e = cudaMalloc((void **)&c->d_slab, c->slab_bytes);
     if (e != cudaSuccess) { delete c; return gcm_cuda_fail(e); }
     c->d_te0 = (uint32_t *)(c->d_slab + o_te0);
     c->d_rk = (uint32_t *)(c->d_slab + o_rk);
@@ -107,8 +158,8 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
 
     int rc = GCM_OK;
     do {
-        if ((e = cudaHostAlloc((void **)&c->h_pinned, 64, cudaHostAllocMapped)) != cudaSuccess) break;
-        if ((e = cudaMemset(c->d_slab, 0, c->slab_bytes)) != cudaSuccess) break;
+        if ((c->h_pinned = pin_take()) == nullptr) { e = cudaErrorMemoryAllocation; break; }
+        if ((e = cudaMemsetAsync(c->d_slab, 0, c->slab_bytes, 0)) != cudaSuccess) break;
         SetupParams sp = setup_params(c, key);
         launch_setup(sp, 0);
         secure_zero(&sp, sizeof(sp));
@@ -129,18 +180,41 @@ extern "C" void gcm_destroy(gcm_ctx *c)
     if (!c) return;
     cudaSetDevice(c->device);
     gcm_host_pipe_free(c);
+    bool pooled = false;
     if (c->d_slab) {
-        launch_wipe(c->d_slab, c->slab_bytes, nullptr, 0);
+        launch_wipe(c->d_slab, c->slab_bytes, nullptr, 0);      // key material never outlives the context
         cudaDeviceSynchronize();
-        cudaFree(c->d_slab);
     }
     if (c->h_pinned) {
         secure_zero(c->h_pinned, 64);
-        cudaFreeHost(c->h_pinned);
+        pin_give(c->h_pinned);
     }
+    if (c->d_slab && cudaGetLastError() == cudaSuccess) {
+        std::lock_guard<std::mutex> lock(g_pool_mu);
+        if (g_pool.size() < kPoolMax) {
+            g_pool.push_back(PooledSlab{c->device, c->d_slab, c->slab_bytes});
+            pooled = true;
+        }
+    }
+    if (!pooled && c->d_slab) cudaFree(c->d_slab);
     cudaGetLastError();
     secure_zero(c, sizeof(*c));
     delete c;
+}
+
+void gcm_pool_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    for (const PooledSlab &p : g_pool) {           // already wiped when they were pooled
+        cudaSetDevice(p.device);
+        cudaFree(p.d_slab);
+    }
+    g_pool.clear();
+    if (g_pin_page && g_pin_used == 0) {
+        cudaFreeHost(g_pin_page);
+        g_pin_page = nullptr;
+    }
+    cudaGetLastError();
 }
 
 extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)

@@ -40,3 +40,5 @@ void gcm_host_pipe_free(gcm_ctx *c);
 int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
                  const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream,
                  unsigned long long *d_sum32);
+// gcm_api.cu: frees the pooled (wiped) allocations of destroyed contexts.
+void gcm_pool_release(void);

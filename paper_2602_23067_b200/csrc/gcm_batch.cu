@@ -609,6 +609,7 @@ extern "C" void gcm_batch_release(void)
     std::lock_guard<std::mutex> lock(g.mu);
     evict_keys_locked();
     free_staging_locked();
+    gcm_pool_release();
 }
 
 extern "C" int gcm_encrypt_batch(gcm_msg *msgs, uint32_t n, void *stream) { return run_batch(msgs, n, stream, false); }
