@@ -20,9 +20,16 @@
 #include "gcm_api_internal.h"
 #include "fits_sum.cuh"
 
+#ifndef PIPE_SLOTS
 #define PIPE_SLOTS 3
+#endif
 #define PIPE_CHUNK_BYTES (64ull << 20)   /* staging buffer = largest chunk; multiple of 16 */
+#ifndef PIPE_MIN_CHUNK_BYTES
 #define PIPE_MIN_CHUNK_BYTES (4ull << 20)
+#endif
+#ifndef PIPE_TARGET_CHUNKS
+#define PIPE_TARGET_CHUNKS 8
+#endif
 
 struct HostPipe {
     cudaStream_t stream[PIPE_SLOTS];
@@ -123,7 +130,7 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
 
     // about eight chunks per message so that H2D, kernel and D2H of neighbouring chunks overlap also for
     // FITS-sized (tens of MiB) messages; 4 MiB at least (launch and table-fill cost), 64 MiB at most (staging)
-    uint64_t chunk = ((len / 8 + (1ull << 20) - 1) >> 20) << 20;
+    uint64_t chunk = ((len / PIPE_TARGET_CHUNKS + (1ull << 20) - 1) >> 20) << 20;
     if (chunk < PIPE_MIN_CHUNK_BYTES) chunk = PIPE_MIN_CHUNK_BYTES;
     if (chunk > PIPE_CHUNK_BYTES) chunk = PIPE_CHUNK_BYTES;
     const uint64_t n_chunks = len ? (len + chunk - 1) / chunk : 1;
