@@ -205,3 +205,31 @@ def test_config_c5_full(G, oracle):
         assert not bool(d_back.any().item())
     finally:
         G.gcm_destroy(ctx)
+
+
+def test_beyond_4gib_ragged(G, oracle):
+    """Maximum-size edge of the single-message path that C5 does not reach: byte offsets above 2^32 and block
+    indices above 2^28 (64-bit offsets, 32-bit counters), with a ragged 13-byte tail.  Every ciphertext byte and
+    the tag against the oracle, then the round trip."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 14 << 30:
+        pytest.skip("needs 14 GiB of free device memory")
+    n = (4 << 30) + (32 << 20) + 13
+    m = workloads.config_c5(payload_bytes=16, with_payload=False)     # key, IV and header AAD of the C5 recipe
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(77)
+    d_pt = torch.randint(-2 ** 63, 2 ** 63 - 1, ((n + 7) // 8,), dtype=torch.int64, device="cuda", generator=gen).view(torch.uint8)[:n]
+    d_ct = torch.empty(n, dtype=torch.uint8, device="cuda")
+    d_aad = dev(m.aad[:777])                                   # AAD that is not a whole number of blocks
+    ctx = G.gcm_init(m.key)
+    try:
+        tag = G.gcm_encrypt(ctx, m.iv, d_aad, d_pt, d_ct)
+        oracle_check_device_message(oracle, m.key, m.iv, m.aad[:777], d_pt, d_ct, tag, "4 GiB + 32 MiB + 13")
+        d_back = torch.empty(n, dtype=torch.uint8, device="cuda")
+        assert G.gcm_decrypt_verify(ctx, m.iv, d_aad, d_ct, d_back, tag) == G.GCM_OK
+        assert torch.equal(d_back, d_pt)
+        d_ct[n - 1] ^= 0x40                                    # last (partial-block) byte, above 2^32
+        assert G.gcm_decrypt_verify(ctx, m.iv, d_aad, d_ct, d_back, tag) == G.GCM_ERR_AUTH
+        assert not bool(d_back.any().item())
+    finally:
+        G.gcm_destroy(ctx)
