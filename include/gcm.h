@@ -83,7 +83,9 @@ GCM_API void gcm_destroy(gcm_ctx *ctx);
  * Launch geometry of the fused kernel: `grid` CTAs (0 = one per SM) of `threads` threads (256, 384
  * or 512; 0 = default 512).  The stride power H^(grid*threads) and its table are rebuilt.  Results
  * never depend on the geometry (geometry-agnostic counters; reading S11).
- * Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
+ * Under the default geometry, messages of at most 511 GHASH blocks (AAD blocks + payload blocks + the length
+ * block, about 8 KiB) take a single-CTA latency kernel instead; an explicit geometry always selects the
+ * fused kernel.  Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
  */
 GCM_API int gcm_set_geometry(gcm_ctx *ctx, int grid, int threads);
 GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);

@@ -309,6 +309,17 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     return GCM_OK;
 }
 
+// Header-sized messages take the single-CTA latency kernel (gcm_small.cu) under the default geometry; an
+// explicit gcm_set_geometry always selects the fused kernel (the geometry tests rely on that).
+static cudaError_t launch_auto(gcm_ctx *c, int mode, int blocks, const GcmParams &p, cudaStream_t s)
+{
+    const uint64_t n_ghash = (uint64_t)p.n_aad_blocks + (p.len + 15) / 16 + 1;
+    if (mode != MODE_GHASH && n_ghash <= SMALL_MAX_BLOCKS && c->grid == c->sm_count && c->threads == GCM_MAX_THREADS &&
+        !p.chain_in && !p.chain_out)
+        return launch_small(c->nr, mode, p, s);
+    return launch_fused(c->nr, mode, c->threads, blocks, p, s);
+}
+
 extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
                                  const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
 {
@@ -319,7 +330,7 @@ extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_tag;
     CU(cudaSetDevice(c->device));
-    cudaError_t e = launch_fused(c->nr, MODE_ENCRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    cudaError_t e = launch_auto(c, MODE_ENCRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;
@@ -337,7 +348,7 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
     p.tag_in = (const uint4 *)d_tag;
     p.status = (int *)d_status;
     CU(cudaSetDevice(c->device));
-    cudaError_t e = launch_fused(c->nr, MODE_DECRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    cudaError_t e = launch_auto(c, MODE_DECRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     // validation gate + payload suppression (L243), decided on the device
@@ -386,7 +397,7 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
     memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
     p.status = (int *)(c->h_pinned + 16);   // verdict written straight into mapped pinned host memory
     CU(cudaSetDevice(c->device));
-    cudaError_t e = launch_fused(c->nr, MODE_DECRYPT, c->threads, blocks, p, (cudaStream_t)stream);
+    cudaError_t e = launch_auto(c, MODE_DECRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     CU(cudaStreamSynchronize((cudaStream_t)stream));

@@ -5,3 +5,8 @@
 
 // nr: 10 or 14; mode: MODE_*; threads: 256 or 512; blocks: CTAs to launch
 cudaError_t launch_fused(int nr, int mode, int threads, int blocks, const GcmParams &p, cudaStream_t s);
+
+// gcm_small.cu: single-CTA latency kernel for messages of at most SMALL_MAX_BLOCKS GHASH blocks
+// (AAD blocks + payload blocks + the length block); MODE_ENCRYPT / MODE_DECRYPT only, no chunk chaining.
+#define SMALL_MAX_BLOCKS 511
+cudaError_t launch_small(int nr, int mode, const GcmParams &p, cudaStream_t s);

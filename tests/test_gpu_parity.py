@@ -117,6 +117,75 @@ def test_many_lengths_small_geometry(G, oracle):
         G.gcm_destroy(ctx)
 
 
+@pytest.mark.parametrize("klen", [16, 32])
+def test_latency_kernel_every_shape(G, oracle, klen):
+    """Messages of at most 511 GHASH blocks take the single-CTA latency kernel (gcm_small.cu) under the default
+    geometry: every payload length 0..130, AAD lengths around block edges, the boundary to the fused kernel
+    (510, 511, 512 blocks), unaligned and in-place buffers with guard regions, and every tamper kind."""
+    rng = np.random.default_rng(9350 + klen)
+    key = rnd(rng, klen).tobytes()
+    ctx = G.gcm_init(key)
+    try:
+        for n in range(0, 131):
+            a = (0, 1, 15, 16, 17, 33, 256)[n % 7]
+            check_message(G, oracle, ctx, key, rnd(rng, 12).tobytes(), rnd(rng, a), rnd(rng, n), "len=%d aad=%d" % (n, a))
+        for blocks, a in [(508, 16), (509, 16), (510, 16), (509, 0), (510, 0), (511, 0), (329, 2880), (330, 2880), (331, 2871)]:
+            for tail in (0, 5):
+                n = 16 * blocks - tail
+                check_message(G, oracle, ctx, key, rnd(rng, 12).tobytes(), rnd(rng, a), rnd(rng, n), "blocks=%d aad=%d" % (blocks, a))
+        # unaligned input / output / AAD, nothing written outside the output range
+        iv, aad, n = rnd(rng, 12).tobytes(), rnd(rng, 45), 16 * 200 + 9
+        pt = rnd(rng, n)
+        ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+        for (oi, oo, oa) in [(0, 0, 0), (1, 0, 0), (0, 3, 0), (5, 5, 1), (15, 9, 7)]:
+            big_in = torch.zeros(n + 64, dtype=torch.uint8, device="cuda")
+            big_out = torch.zeros(n + 64, dtype=torch.uint8, device="cuda")
+            big_aad = torch.zeros(len(aad) + 16, dtype=torch.uint8, device="cuda")
+            big_in[oi: oi + n] = dev(pt)
+            big_aad[oa: oa + len(aad)] = dev(aad)
+            tag = G.gcm_encrypt(ctx, iv, big_aad[oa: oa + len(aad)], big_in[oi: oi + n], big_out[oo: oo + n])
+            out = big_out.cpu().numpy()
+            assert tag == ref_tag and np.array_equal(out[oo: oo + n], ref_ct), (oi, oo, oa)
+            assert not out[:oo].any() and not out[oo + n:].any(), "wrote outside the output range"
+        buf = dev(pt).clone()
+        assert G.gcm_encrypt(ctx, iv, dev(aad), buf, buf) == ref_tag and np.array_equal(buf.cpu().numpy(), ref_ct)   # in place
+        assert G.gcm_decrypt_verify(ctx, iv, dev(aad), buf, buf, ref_tag) == G.GCM_OK
+        assert np.array_equal(buf.cpu().numpy(), pt)
+        # tamper: ciphertext, tag, AAD, IV, length -> GCM_ERR_AUTH and an all-zero output
+        d_aad, d_ct = dev(aad), dev(ref_ct)
+
+        def rejected(iv_=iv, aad_=d_aad, ct_=d_ct, tag_=ref_tag):
+            out = torch.full((ct_.numel(),), 0xAA, dtype=torch.uint8, device="cuda")
+            return G.gcm_decrypt_verify(ctx, iv_, aad_, ct_, out, tag_) == G.GCM_ERR_AUTH and not bool(out.any().item())
+
+        for pos in (0, n // 2, n - 1):
+            bad = d_ct.clone(); bad[pos] ^= 0x10
+            assert rejected(ct_=bad)
+        t = bytearray(ref_tag); t[15] ^= 0x80
+        assert rejected(tag_=bytes(t))
+        bad_aad = d_aad.clone(); bad_aad[44] ^= 1
+        assert rejected(aad_=bad_aad) and rejected(aad_=d_aad[:-1].clone()) and rejected(ct_=d_ct[:-1].clone())
+        v = bytearray(iv); v[0] ^= 2
+        assert rejected(iv_=bytes(v))
+        # async form on the latency kernel: device tag in, status word out, gated wipe
+        d_tag = dev(np.frombuffer(ref_tag, np.uint8))
+        d_status = torch.full((1,), -7, dtype=torch.int32, device="cuda")
+        out = torch.full((n,), 0x55, dtype=torch.uint8, device="cuda")
+        bad = d_ct.clone(); bad[3] ^= 1
+        G.gcm_decrypt_verify_async(ctx, iv, d_aad, bad, out, d_tag, d_status)
+        torch.cuda.synchronize()
+        assert int(d_status.item()) == G.GCM_ERR_AUTH and not bool(out.any().item())
+        G.gcm_decrypt_verify_async(ctx, iv, d_aad, d_ct, out, d_tag, d_status)
+        torch.cuda.synchronize()
+        assert int(d_status.item()) == G.GCM_OK and np.array_equal(out.cpu().numpy(), pt)
+        # the same messages through the fused kernel (explicit geometry) give the same bytes
+        G.gcm_set_geometry(ctx, 3, 256)
+        d_out = torch.empty(n, dtype=torch.uint8, device="cuda")
+        assert G.gcm_encrypt(ctx, iv, d_aad, dev(pt), d_out) == ref_tag and np.array_equal(d_out.cpu().numpy(), ref_ct)
+    finally:
+        G.gcm_destroy(ctx)
+
+
 def test_in_place_and_unaligned(G, oracle):
     rng = np.random.default_rng(9400)
     key = rnd(rng, 32).tobytes()
