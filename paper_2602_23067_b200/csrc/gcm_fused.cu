@@ -52,12 +52,6 @@ __device__ __forceinline__ uint4 warp_h_power(const uint4 *hx, uint64_t d, uint3
     return f;
 }
 
-#ifdef GCM_PHASE_PROBE      // _work latency probe only: clock64 stamps of CTA 0 / thread 0 behind the partials
-#define STAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) ((long long *)(p.partials + 4000))[i] = clock64(); } while (0)
-#else
-#define STAMP(i) do { } while (0)
-#endif
-
 template <int NR, int MODE, int TPB>
 __global__ void __launch_bounds__(TPB, 1)
 gcm_fused_kernel(const __grid_constant__ GcmParams p)
@@ -78,7 +72,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     const uint32_t r0 = r0_64 < S ? (uint32_t)r0_64 : S;
     const uint32_t r1 = (uint64_t)r0 + Q < S ? r0 + Q : S;
     const bool has_rows = r0 < r1;
-    STAMP(0);
 
     {
         KtabRegs<TPB> kr;
@@ -91,7 +84,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     const bool tail_warp = has_rows && r1 == S;          // owns the last (possibly ragged) row
     if (has_rows && !tail_warp) wpow = warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane, p.vblocks);
     __syncthreads();
-    STAMP(1);
 
     uint32_t sel[8];
 #pragma unroll
@@ -158,8 +150,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         }
         if (fast || valid) Y = xor4(ym, X);
     }
-
-    STAMP(2);
     // a8: lane correction H^(blocks from the lane's last block to the end of the warp's run), XOR over
     // the warp, warp correction H^(blocks behind the run), XOR over the CTA.  In the ragged last row
     // only lanes < rem folded a block; rotating the lane order by rem keeps the exponents in 1..32.
@@ -185,7 +175,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
         }
     }
-    STAMP(3);
     // a9: last-CTA-done combination of the partials
     if (t == 0) {
         p.partials[blockIdx.x] = part;
@@ -195,7 +184,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     }
     __syncthreads();
     if (!s_last) return;
-    STAMP(4);
     __threadfence();
     uint4 acc = make_uint4(0, 0, 0, 0);
     for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
@@ -227,7 +215,6 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
             }
         }
         *p.counter = 0;   // ready for the next launch on this context
-        STAMP(5);
     }
 }
 
