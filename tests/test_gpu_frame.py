@@ -65,7 +65,8 @@ def test_access_scenarios_match_oracle(gfc, F, ctx, spec):
 
 def test_tamper_matches_oracle(gfc, F, ctx):
     f = workloads.fits_frame(seed=2005, ny=64, nx=96, n_sources=4)
-    c = gfc.gfc_encrypt_frame(ctx, f.fits, f.key_h, f.key_d, f.nonce_h, f.nonce_d).tobytes()
+    c = F.encrypt_frame(f.fits, f.key_h, f.key_d, f.nonce_h, f.nonce_d)          # oracle-written; the CUDA path must agree
+    assert gfc.gfc_encrypt_frame(ctx, f.fits, f.key_h, f.key_d, f.nonce_h, f.nonce_d).tobytes() == c
     cases = []
     pos = c.index(b"ORIG_NA1=") + 29                      # last digit of the value
     cases.append(c[:pos] + bytes([c[pos] ^ 1]) + c[pos + 1:])
@@ -131,10 +132,15 @@ def test_errors_and_random_nonces(gfc, F, ctx):
         assert e.value.code == gfc.GFC_ERR_CAPACITY
     finally:
         gfc.gfc_context_destroy(small)
-    # nonces from the OS entropy pool (L137): two containers of the same file differ, both open in the oracle
+    # nonces from the OS entropy pool (L137): two containers of the same file differ; with the nonces the library
+    # drew (read back from the NONCE_H / NONCE_D cards, they are inputs) the oracle writes the same bytes
     a = gfc.gfc_encrypt_frame(ctx, f.fits, f.key_h, f.key_d).tobytes()
     b = gfc.gfc_encrypt_frame(ctx, f.fits, f.key_h, f.key_d).tobytes()
     assert a != b
     for c in (a, b):
-        out, warn = F.decrypt_frame(c, f.key_h, f.key_d)
-        assert warn == 0 and out == f.fits
+        nh = bytes.fromhex(c[c.index(b"NONCE_H = '") + 11:][:24].decode())
+        nd = bytes.fromhex(c[c.index(b"NONCE_D = '") + 11:][:24].decode())
+        assert nh != f.nonce_h and nd != f.nonce_d and nh != nd
+        assert c == F.encrypt_frame(f.fits, f.key_h, f.key_d, nh, nd)
+        back = gfc.gfc_decrypt_frame(ctx, c, f.key_h, f.key_d)
+        assert back.warning_code == 0 and back.tobytes() == f.fits

@@ -254,7 +254,9 @@ def test_tamper_detection_and_suppression(G, oracle, klen):
         assert rejected(ct_=d_ct[:-1].clone())
         # the oracle agrees on rejection and on zeros
         bad = d_ct.clone(); bad[7] ^= 0x80
-        rc, out = oracle.gcm_decrypt_verify(key, iv, aad, bad.cpu().numpy(), tag)
+        ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)     # the oracle's own ciphertext, same flip
+        ref_bad = ref_ct.copy(); ref_bad[7] ^= 0x80
+        rc, out = oracle.gcm_decrypt_verify(key, iv, aad, ref_bad, ref_tag)
         assert rc == oracle.AUTH_FAIL and not out.any()
         # async form: status word + wipe kernel on the stream
         d_tag = dev(np.frombuffer(tag, np.uint8))
