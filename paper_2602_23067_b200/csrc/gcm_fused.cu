@@ -79,10 +79,7 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
         ktab_store<TPB>(kr, sm);
     }
-    // position weight of the warp's run, H^(blocks behind it): computed while the tables arrive
-    uint4 wpow = make_uint4(0, 0, 0, 0);
     const bool tail_warp = has_rows && r1 == S;          // owns the last (possibly ragged) row
-    if (has_rows && !tail_warp) wpow = warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane, p.vblocks);
     __syncthreads();
 
     uint32_t sel[8];
@@ -105,7 +102,21 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     uint4 pre = make_uint4(0, 0, 0, 0);
     bool have_pre = false;
 
+    // a8, first half: the weight each lane's partial is multiplied by at the end of the run,
+    //     V_l = H^(blocks from the lane's last block to the end of the run) . H^(blocks behind the run).
+    // In the ragged last row only lanes < rem folded a block; rotating the lane order by rem keeps the first
+    // exponent in 1..32.  The generic products behind V (up to three per warp) are NOT done before the rows or
+    // after them, where all warps of the SM would do them at once with the table pipe idle, but in the middle
+    // of the run, at a row that differs from warp to warp: the other warps keep the shared-memory pipe busy.
+    uint4 V = make_uint4(0, 0, 0, 0);
+    const uint32_t rmid = r0 + (uint32_t)(((uint64_t)(r1 - r0) * (warp + 1)) / (TPB / 32 + 1));
+
     for (uint32_t row = r0; row < r1; row++) {
+        if (row == rmid) {                               // once per run, at a warp-specific row (see above)
+            const uint32_t rem = tail_warp ? (uint32_t)(p.vblocks - 32ull * (S - 1)) : 32u;   // 1..32
+            V = __ldg(p.tab.hpow + (((rem - lane - 1) & 31) + 1));
+            if (!tail_warp) V = gf_mul_mem(V, warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane, p.vblocks));
+        }
         const uint64_t v = 32ull * row + lane;          // virtual block index
         const bool fast = row >= p.fast_lo && row < p.fast_hi;
         uint4 x = make_uint4(0, 0, 0, 0);
@@ -150,21 +161,14 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
         }
         if (fast || valid) Y = xor4(ym, X);
     }
-    // a8: lane correction H^(blocks from the lane's last block to the end of the warp's run), XOR over
-    // the warp, warp correction H^(blocks behind the run), XOR over the CTA.  In the ragged last row
-    // only lanes < rem folded a block; rotating the lane order by rem keeps the exponents in 1..32.
+    // a8, second half: one product per lane, XOR over the warp, XOR over the CTA
     uint4 part = make_uint4(0, 0, 0, 0);
-    if (has_rows) {
-        const uint32_t rem = tail_warp ? (uint32_t)(p.vblocks - 32ull * (S - 1)) : 32u;   // 1..32
-        const uint32_t e = ((rem - lane - 1) & 31) + 1;
-        part = gf_mul_mem(Y, __ldg(p.tab.hpow + e));
-    }
+    if (has_rows) part = gf_mul_mem(Y, V);
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) {
         part.x ^= __shfl_xor_sync(0xFFFFFFFFu, part.x, o); part.y ^= __shfl_xor_sync(0xFFFFFFFFu, part.y, o);
         part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
     }
-    if (has_rows && !tail_warp) part = gf_mul_mem(part, wpow);
     if (lane == 0) red[warp] = part;
     __syncthreads();
     if (warp == 0) {
