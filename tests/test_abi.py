@@ -65,3 +65,21 @@ def test_no_cpu_fallback_in_product_path():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text, f
                 assert "liboracle" not in text, f
+
+
+def test_headers_are_plain_c(tmp_path):
+    """The boundary is a C ABI: both headers must compile as C11 with no C++ and no CUDA or torch types."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "use.c"
+    src.write_text('#include "gcm.h"\n#include "gfc.h"\n'
+                   "int main(void) { gcm_msg m; FitsOperationResult r; (void)m; (void)r;\n"
+                   "  return (int)sizeof(m) + (int)sizeof(r) + GCM_ERR_AUTH + GFC_ERR_FORMAT + GCM_RATE_COUNT > 0 ? 0 : 1; }\n")
+    subprocess.run([gcc, "-std=c11", "-Wall", "-Werror", "-pedantic", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), str(src)],
+                   check=True)
+    for h in ("gcm.h", "gfc.h"):
+        text = open(os.path.join(ROOT, "include", h)).read()
+        assert "#include <cuda" not in text and "#include <torch" not in text and "at::Tensor" not in text, h
