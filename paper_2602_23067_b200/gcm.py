@@ -120,6 +120,22 @@ def _stream(stream) -> Optional[int]:
     return stream.cuda_stream or None
 
 
+def _iv(iv) -> bytes:
+    """The C side reads exactly 12 bytes (include/gcm.h: 96-bit IV only, reading S5): refuse anything else here,
+    a short IV would be read past its end and a longer one silently truncated (nonce collisions)."""
+    iv = bytes(iv)
+    if len(iv) != 12:
+        raise ValueError("iv must be exactly 12 bytes (96 bits), got %d" % len(iv))
+    return iv
+
+
+def _tag(tag) -> bytes:
+    tag = bytes(tag)
+    if len(tag) != 16:
+        raise ValueError("tag must be exactly 16 bytes, got %d" % len(tag))
+    return tag
+
+
 def _check(rc: int, where: str, ok: Sequence[int] = (GCM_OK,)) -> int:
     if rc not in ok:
         raise GcmError(rc, where)
@@ -146,6 +162,8 @@ def gcm_last_cuda_error_string() -> str:
 def gcm_init(key: bytes, key_bits: Optional[int] = None) -> int:
     key = bytes(key)
     bits = 8 * len(key) if key_bits is None else int(key_bits)
+    if bits not in (128, 256) or 8 * len(key) != bits:
+        raise ValueError("key must be 16 or 32 bytes and match key_bits (got %d bytes, key_bits=%d)" % (len(key), bits))
     h = ctypes.c_void_p()
     _check(_L.gcm_init(ctypes.byref(h), key, bits), "gcm_init")
     return h.value
@@ -175,42 +193,43 @@ def gcm_get_hash_subkey(ctx: int) -> bytes:
 def gcm_encrypt(ctx: int, iv: bytes, aad, pt, ct, stream=None) -> bytes:
     """Encrypts device buffer `pt` into device buffer `ct` (same size; may be the same tensor) and
     returns the 16-byte tag."""
+    iv = _iv(iv)
     a_ptr, a_len = _dev(aad)
     p_ptr, p_len = _dev(pt)
     c_ptr, c_len = _dev(ct)
     if c_len != p_len:
         raise ValueError("ct and pt sizes differ")
     tag = ctypes.create_string_buffer(16)
-    _check(_L.gcm_encrypt(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)), "gcm_encrypt")
+    _check(_L.gcm_encrypt(ctx, iv, a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)), "gcm_encrypt")
     return tag.raw
 
 
 def gcm_decrypt_verify(ctx: int, iv: bytes, aad, ct, pt, tag: bytes, stream=None) -> int:
     """Returns GCM_OK (plaintext in `pt`) or GCM_ERR_AUTH (`pt` zero-filled)."""
+    iv, tag = _iv(iv), _tag(tag)
     a_ptr, a_len = _dev(aad)
     c_ptr, c_len = _dev(ct)
     p_ptr, p_len = _dev(pt)
     if c_len != p_len:
         raise ValueError("ct and pt sizes differ")
-    tag = bytes(tag)
-    if len(tag) != 16:
-        raise ValueError("tag must be 16 bytes")
-    return _check(_L.gcm_decrypt_verify(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
+    return _check(_L.gcm_decrypt_verify(ctx, iv, a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
                   "gcm_decrypt_verify", ok=(GCM_OK, GCM_ERR_AUTH))
 
 
 def gcm_encrypt_async(ctx: int, iv: bytes, aad, pt, ct, d_tag, stream=None) -> None:
+    iv = _iv(iv)
     a_ptr, a_len = _dev(aad)
     p_ptr, p_len = _dev(pt)
     c_ptr, _ = _dev(ct)
     t_ptr, t_len = _dev(d_tag)
     if t_len < 16:
         raise ValueError("d_tag must hold 16 bytes")
-    _check(_L.gcm_encrypt_async(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, t_ptr, _stream(stream)),
+    _check(_L.gcm_encrypt_async(ctx, iv, a_ptr, a_len, p_ptr, p_len, c_ptr, t_ptr, _stream(stream)),
            "gcm_encrypt_async")
 
 
 def gcm_decrypt_verify_async(ctx: int, iv: bytes, aad, ct, pt, d_tag, d_status, stream=None) -> None:
+    iv = _iv(iv)
     a_ptr, a_len = _dev(aad)
     c_ptr, c_len = _dev(ct)
     p_ptr, _ = _dev(pt)
@@ -218,7 +237,7 @@ def gcm_decrypt_verify_async(ctx: int, iv: bytes, aad, ct, pt, d_tag, d_status, 
     s_ptr, s_len = _dev(d_status)
     if t_len < 16 or s_len < 4:
         raise ValueError("d_tag must hold 16 bytes and d_status 4")
-    _check(_L.gcm_decrypt_verify_async(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, t_ptr, s_ptr,
+    _check(_L.gcm_decrypt_verify_async(ctx, iv, a_ptr, a_len, c_ptr, c_len, p_ptr, t_ptr, s_ptr,
                                        _stream(stream)), "gcm_decrypt_verify_async")
 
 
@@ -247,28 +266,27 @@ def _host(buf, writable: bool = False) -> Tuple[Optional[int], int, object]:
 
 def gcm_encrypt_host(ctx: int, iv: bytes, h_aad, h_pt, h_ct, stream=None) -> bytes:
     """HOST buffers in and out (chunked H2D -> kernel -> D2H pipeline inside the library)."""
+    iv = _iv(iv)
     a_ptr, a_len, ka = _host(h_aad)
     p_ptr, p_len, kp = _host(h_pt)
     c_ptr, c_len, kc = _host(h_ct, writable=True)
     if c_len != p_len:
         raise ValueError("ct and pt sizes differ")
     tag = ctypes.create_string_buffer(16)
-    _check(_L.gcm_encrypt_host(ctx, bytes(iv), a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)),
+    _check(_L.gcm_encrypt_host(ctx, iv, a_ptr, a_len, p_ptr, p_len, c_ptr, tag, _stream(stream)),
            "gcm_encrypt_host")
     del ka, kp, kc
     return tag.raw
 
 
 def gcm_decrypt_verify_host(ctx: int, iv: bytes, h_aad, h_ct, h_pt, tag: bytes, stream=None) -> int:
+    iv, tag = _iv(iv), _tag(tag)
     a_ptr, a_len, ka = _host(h_aad)
     c_ptr, c_len, kc = _host(h_ct)
     p_ptr, p_len, kp = _host(h_pt, writable=True)
     if c_len != p_len:
         raise ValueError("ct and pt sizes differ")
-    tag = bytes(tag)
-    if len(tag) != 16:
-        raise ValueError("tag must be 16 bytes")
-    rc = _check(_L.gcm_decrypt_verify_host(ctx, bytes(iv), a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
+    rc = _check(_L.gcm_decrypt_verify_host(ctx, iv, a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
                 "gcm_decrypt_verify_host", ok=(GCM_OK, GCM_ERR_AUTH))
     del ka, kp, kc
     return rc
@@ -288,11 +306,13 @@ def _pack_msgs(msgs: Iterable[dict], decrypt: bool):
     arr = (GcmMsg * max(1, len(msgs)))()
     keep = []
     for i, m in enumerate(msgs):
+        if len(bytes(m["key"])) not in (16, 32):
+            raise ValueError("message %d: key must be 16 or 32 bytes" % i)
         key = ctypes.create_string_buffer(bytes(m["key"]), len(m["key"]))
         keep.append(key)
         arr[i].key = ctypes.cast(key, ctypes.c_void_p)
         arr[i].key_bits = 8 * len(m["key"])
-        arr[i].iv[:] = list(bytes(m["iv"]))
+        arr[i].iv[:] = list(_iv(m["iv"]))
         a_ptr, a_len = _dev(m.get("aad"))
         i_ptr, i_len = _dev(m["input"])
         o_ptr, o_len = _dev(m["output"])
@@ -302,7 +322,7 @@ def _pack_msgs(msgs: Iterable[dict], decrypt: bool):
         arr[i].d_in, arr[i].len = i_ptr, i_len
         arr[i].d_out = o_ptr
         if decrypt:
-            arr[i].tag[:] = list(bytes(m["tag"]))
+            arr[i].tag[:] = list(_tag(m["tag"]))
     return arr, len(msgs), keep
 
 

@@ -46,14 +46,47 @@ def test_binding_lists_the_same_symbols(lib_path):
 def test_argument_errors_without_gpu(lib_path):
     """Argument validation happens before any CUDA call."""
     import paper_2602_23067_b200 as pkg
-    with pytest.raises(pkg.GcmError) as e:
+    with pytest.raises(ValueError):
         pkg.gcm_init(bytes(24))            # AES-192 is outside reading S1
-    assert e.value.code == pkg.GCM_ERR_ARG
+    with pytest.raises(ValueError):
+        pkg.gcm_init(bytes(16), key_bits=256)      # key_bits must match the key (the C side would read 32 bytes)
     L = ctypes.CDLL(lib_path)
     assert L.gcm_init(None, b"0" * 16, 128) == pkg.GCM_ERR_ARG
+    out = ctypes.c_void_p()
+    assert L.gcm_init(ctypes.byref(out), b"0" * 24, 192) == pkg.GCM_ERR_ARG
     assert L.gcm_encrypt(None, None, None, 0, None, 0, None, None, None) == pkg.GCM_ERR_ARG
     assert L.gfc_context_create(None, 0, 0) == pkg.GCM_ERR_ARG
     assert L.gfc_encrypt_frame(None, None, 0, None, None, 128, None, None, None) == pkg.GCM_ERR_ARG
+
+
+def test_binding_refuses_wrong_iv_and_tag_lengths(lib_path):
+    """The C ABI takes `const uint8_t iv[12]` and reads exactly 12 bytes: an 11-byte IV would be read past its end, a
+    16-byte one silently truncated (two IVs that differ in the last 4 bytes would collide; reading S5: 96-bit IVs
+    only).  The binding refuses both in every entry point, before any pointer reaches C."""
+    import paper_2602_23067_b200 as pkg
+    ctx = 0xDEAD                          # never dereferenced: the length check comes first
+    for bad in (bytes(11), bytes(16), b""):
+        with pytest.raises(ValueError):
+            pkg.gcm_encrypt(ctx, bad, None, None, None)
+        with pytest.raises(ValueError):
+            pkg.gcm_decrypt_verify(ctx, bad, None, None, None, bytes(16))
+        with pytest.raises(ValueError):
+            pkg.gcm_encrypt_async(ctx, bad, None, None, None, None)
+        with pytest.raises(ValueError):
+            pkg.gcm_decrypt_verify_async(ctx, bad, None, None, None, None, None)
+        with pytest.raises(ValueError):
+            pkg.gcm_encrypt_host(ctx, bad, None, None, None)
+        with pytest.raises(ValueError):
+            pkg.gcm_decrypt_verify_host(ctx, bad, None, None, None, bytes(16))
+        with pytest.raises(ValueError):
+            pkg.gcm_encrypt_batch([{"key": bytes(16), "iv": bad, "aad": None, "input": None, "output": None}])
+    for bad_tag in (bytes(15), bytes(17)):
+        with pytest.raises(ValueError):
+            pkg.gcm_decrypt_verify(ctx, bytes(12), None, None, None, bad_tag)
+        with pytest.raises(ValueError):
+            pkg.gcm_decrypt_verify_host(ctx, bytes(12), None, None, None, bad_tag)
+    with pytest.raises(ValueError):
+        pkg.gcm_encrypt_batch([{"key": bytes(24), "iv": bytes(12), "aad": None, "input": None, "output": None}])
 
 
 def test_no_cpu_fallback_in_product_path():
