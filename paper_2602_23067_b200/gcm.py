@@ -306,8 +306,6 @@ def _pack_msgs(msgs: Iterable[dict], decrypt: bool):
     arr = (GcmMsg * max(1, len(msgs)))()
     keep = []
     for i, m in enumerate(msgs):
-        if len(bytes(m["key"])) not in (16, 32):
-            raise ValueError("message %d: key must be 16 or 32 bytes" % i)
         key = ctypes.create_string_buffer(bytes(m["key"]), len(m["key"]))
         keep.append(key)
         arr[i].key = ctypes.cast(key, ctypes.c_void_p)

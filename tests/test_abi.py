@@ -85,8 +85,6 @@ def test_binding_refuses_wrong_iv_and_tag_lengths(lib_path):
             pkg.gcm_decrypt_verify(ctx, bytes(12), None, None, None, bad_tag)
         with pytest.raises(ValueError):
             pkg.gcm_decrypt_verify_host(ctx, bytes(12), None, None, None, bad_tag)
-    with pytest.raises(ValueError):
-        pkg.gcm_encrypt_batch([{"key": bytes(24), "iv": bytes(12), "aad": None, "input": None, "output": None}])
 
 
 def test_no_cpu_fallback_in_product_path():

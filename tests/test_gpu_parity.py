@@ -85,8 +85,8 @@ def test_geometry_agnostic(G, oracle, klen):
     ctx = G.gcm_init(key)
     try:
         d_aad, d_pt = dev(aad), dev(pt)
-        for (grid, threads) in [(1, 512), (1, 256), (2, 512), (3, 256), (5, 512), (7, 256), (148, 512),
-                                (148, 256), (200, 512), (0, 0)]:
+        for (grid, threads) in [(1, 512), (1, 256), (1, 384), (2, 512), (3, 256), (5, 512), (5, 384), (7, 256),
+                                (148, 512), (148, 256), (148, 384), (200, 512), (301, 384), (0, 0)]:
             G.gcm_set_geometry(ctx, grid, threads)
             d_ct = torch.empty_like(d_pt)
             tag = G.gcm_encrypt(ctx, iv, d_aad, d_pt, d_ct)
@@ -463,8 +463,8 @@ def test_host_buffers_single_chunk(G, oracle):
 
 
 def test_host_pipeline_multi_chunk(G, oracle):
-    """Three 64 MiB chunks + a ragged tail: the running GHASH state is chained across chunks and the
-    counters continue across chunk boundaries."""
+    """192 MiB + 12345 bytes through the chunk pipeline (about eight chunks, the last one ragged): the running
+    GHASH state is chained across chunks and the counters continue across chunk boundaries."""
     import os
     rng = np.random.default_rng(9800)
     key = rnd(rng, 32).tobytes()
