@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-mib", type=float, default=384.0)
     ap.add_argument("--workload", default="c5",
-                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum"],
+                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum", "phases"],
                     help="c5 = the headline (default); the others are the supplementary measurements of DESIGN.md section 10")
     return ap.parse_args()
 
@@ -581,6 +581,66 @@ def run_extra(args):
                     gpu_launches=None, frames=out,
                     config={"workload": "frame: gfc_encrypt_frame / gfc_decrypt_frame (AES-256, dual key) on a 256x256 and a 4096x4096 float32 "
                                         "FITS file in pinned host memory; H2D and D2H inside the timed region (PCIe-bound)"})
+    elif w == "phases":
+        # Where the fixed cost of a launch goes: the fused kernel's own %globaltimer stamps
+        # (gcm_set_phase_stamps) for message sizes around the paper's FITS files, launches back to back on one stream.
+        m = workloads.config_c2(payload_bytes=0)
+        ctx = G.gcm_init(m.key)
+        aad = torch.from_numpy(m.aad).cuda()
+        d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        grid, _ = G.gcm_get_geometry(ctx)
+        stamps = torch.zeros(G.GCM_PHASE_SLOTS * grid, dtype=torch.int64, device="cuda")
+        out = {}
+        for mib in (1, 4, 16, 64, 256):
+            n = mib << 20
+            pt = rand_bytes(n, 100 + mib)
+            ct = torch.empty_like(pt)
+            G.gcm_set_phase_stamps(ctx, None)
+            for _ in range(warm):
+                G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(steps, 20)
+            e0.record(stream)
+            for _ in range(reps):
+                G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            period_us = e0.elapsed_time(e1) * 1e3 / reps
+            # stamps of the LAST of a train of launches (so that its prologue overlaps the previous launch's tail)
+            stamps.zero_()
+            for _ in range(7):
+                G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+            G.gcm_set_phase_stamps(ctx, stamps)
+            G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+            torch.cuda.synchronize()
+            G.gcm_set_phase_stamps(ctx, None)
+            st = stamps.cpu().numpy().reshape(grid, G.GCM_PHASE_SLOTS).astype(np.int64)
+            live = st[st[:, 0] > 0]
+            t0 = live[:, 0].min()
+            names = ["entry", "tables_ready", "after_dep_wait", "rows_done", "partials_in", "ticket", "finished", "weights_done"]
+            ph = {}
+            for k, name in enumerate(names):
+                col = live[:, k]
+                col = col[col > 0]
+                if col.size:
+                    ph[name] = {"min_us": float(col.min() - t0) / 1e3, "mean_us": float(col.mean() - t0) / 1e3,
+                                "max_us": float(col.max() - t0) / 1e3}
+            ph["per_cta_mean_us"] = {
+                "entry_to_weights": float((live[:, 7] - live[:, 0]).mean()) / 1e3,
+                "entry_to_tables": float((live[:, 1] - live[:, 0]).mean()) / 1e3,
+                "tables_to_dep_wait": float((live[:, 2] - live[:, 1]).mean()) / 1e3,
+                "rows": float((live[:, 3] - live[:, 2]).mean()) / 1e3,
+                "lane_products_and_sync": float((live[:, 4] - live[:, 3]).mean()) / 1e3,
+                "cta_combine_and_ticket": float((live[:, 5] - live[:, 4]).mean()) / 1e3,
+            }
+            out["%d_MiB" % mib] = {"launch_period_us": period_us, "GBps": n / period_us / 1e3, "ctas": int(live.shape[0]),
+                                   "first_entry_to_finish_us": ph.get("finished", {}).get("max_us"), "phases": ph}
+        G.gcm_destroy(ctx)
+        line.update(metric="fused kernel phase breakdown (us, %globaltimer stamps of the last of 8 back-to-back launches)",
+                    value=out["16_MiB"]["launch_period_us"], unit="us", higher_is_better=False,
+                    ms_per_step=out["16_MiB"]["launch_period_us"] / 1e3, gpu_launches=None, phases=out,
+                    config={"workload": "phases: AES-256-GCM encrypt of 1 / 4 / 16 / 64 / 256 MiB, 2880-byte AAD, launches back to back; "
+                                        "pdl=%s" % ("off" if os.environ.get("GCM_NO_PDL") else "on")})
     elif w == "latency":
         # single-message latency through the synchronous non-batched call (C4's report): host wall clock
         m = workloads.config_c1(payload_bytes=0)

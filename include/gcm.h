@@ -19,7 +19,10 @@
  *   - In place (out == in) is allowed; any other overlap of in and out is GCM_ERR_ARG.
  *   - Any byte alignment is accepted; the fast path needs `in` and `out` 16-byte aligned.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).
- *   - A gcm_ctx may be used by one call at a time (it owns the cross-CTA scratch of that call).
+ *   - A gcm_ctx may be used by one call at a time (it owns the cross-CTA scratch of that call): a call that
+ *     finds the context in use by another thread returns GCM_ERR_BUSY and does nothing.  Asynchronous calls
+ *     on one context must be issued to one stream (or otherwise ordered) so that their kernels do not overlap.
+ *   - Every call runs on the context's device and leaves the calling thread's current CUDA device as it was.
  *   - On GCM_ERR_AUTH the whole output [0, len) has been overwritten with zeros (the paper's payload
  *     suppression) and the call completes normally (L245).  The fused kernel writes
  *     plaintext before the tag is known (reading S9); the synchronous call does not return before
@@ -50,14 +53,17 @@ enum {
     GCM_ERR_ARG   = -1,  /* NULL pointer, key_bits not 128/256, partial overlap, bad geometry    */
     GCM_ERR_LEN   = -2,  /* len > 2^36 - 32 bytes, or aad_len >= 2^61 bytes                      */
     GCM_ERR_CUDA  = -3,  /* CUDA runtime failure; see gcm_last_cuda_error()                      */
-    GCM_ERR_NOMEM = -4
+    GCM_ERR_NOMEM = -4,
+    GCM_ERR_BUSY  = -5   /* the context is in use by another call                                */
 };
 
 /* Library / build identification: "b200gcm <version> sm_100a". Never NULL. */
 GCM_API const char *gcm_version(void);
 
-/* Selects the CUDA device (ordinal) used by subsequent gcm_init / batch calls of this thread's
- * process.  Default 0.  Returns GCM_OK or GCM_ERR_CUDA. */
+/* Selects the CUDA device (ordinal) on which subsequent gcm_init / batch / gfc_context_create calls of the
+ * process make their contexts; -1 (the default) = the calling thread's current CUDA device at the time of the
+ * call.  Does not change the caller's current device.  A context stays on the device it was made on.
+ * Returns GCM_OK, GCM_ERR_ARG (no such device) or GCM_ERR_CUDA. */
 GCM_API int gcm_set_device(int ordinal);
 
 /* Last cudaError_t seen by the library (0 = none), and its text (host, static storage). */
@@ -80,9 +86,9 @@ GCM_API int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits);
 GCM_API void gcm_destroy(gcm_ctx *ctx);
 
 /*
- * Launch geometry of the fused kernel: `grid` CTAs (0 = one per SM) of `threads` threads (256, 384
- * or 512; 0 = default 512).  The stride power H^(grid*threads) and its table are rebuilt.  Results
- * never depend on the geometry (geometry-agnostic counters; reading S11).
+ * Launch geometry of the fused kernel: at most `grid` CTAs (0 = one per SM) of `threads` threads (256, 384
+ * or 512; 0 = default 512).  No table depends on it (the GHASH stride power is H^32 for every launch shape), and
+ * results never depend on the geometry (geometry-agnostic counters; reading S11).
  * Under the default geometry, messages of at most 511 GHASH blocks (AAD blocks + payload blocks + the length
  * block, about 8 KiB) take a single-CTA latency kernel instead; an explicit geometry always selects the
  * fused kernel.  Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_CUDA.
@@ -108,6 +114,16 @@ enum {
     GCM_RATE_COUNT
 };
 GCM_API int gcm_measure_pipe_rates(double *rates, int n);
+
+/*
+ * Diagnostics: per-phase time stamps of the fused kernel.  d_stamps (device) has room for
+ * 8 x uint64 per CTA of the largest grid used (GCM_PHASE_SLOTS x grid x 8 bytes); while it is set, thread 0 of
+ * every CTA stores %globaltimer (ns) at: [0] kernel entry, [1] tables in shared memory, [2] after
+ * griddepcontrol.wait, [3] its rows done, [4] all warps' partials in, [5] ticket drawn, [6] finisher done (last CTA
+ * only).  NULL switches it off (the default).  Not part of the data path.
+ */
+#define GCM_PHASE_SLOTS 8
+GCM_API int gcm_set_phase_stamps(gcm_ctx *ctx, void *d_stamps);
 
 /* Copies the hash subkey H = E_K(0^128) (16 bytes) to host memory; for tests of step a2. */
 GCM_API int gcm_get_hash_subkey(const gcm_ctx *ctx, uint8_t h[16]);
@@ -163,8 +179,9 @@ GCM_API int gcm_decrypt_verify_async(gcm_ctx *ctx, const uint8_t iv[12],
  * Host-buffer forms (the paper's data plane stages files through pinned host memory and overlaps
  * the transfers with the kernels on CUDA streams): `h_*` are HOST
  * pointers (pinned memory gives full PCIe rate; pageable memory works).  The message is cut into
- * chunks (about eight per message, 4 MiB to 64 MiB each) that travel H2D -> fused kernel -> D2H on three internal streams; the running
- * GHASH state is handed from chunk to chunk on the device.  Work already queued on `cuda_stream`
+ * chunks (about eight per message, 4 MiB to 64 MiB each) that travel H2D -> fused kernel -> D2H on three internal
+ * streams; the running GHASH state is handed from chunk to chunk on the device.  The plaintext of chunk k is copied
+ * out before the tag of the whole message is known (reading S9); gcm_decrypt_verify_host_strict does not do that.  Work already queued on `cuda_stream`
  * is waited for; the call returns when the output and the tag / verdict are in host memory.
  * On GCM_ERR_AUTH h_pt[0..len) is zero-filled.  aad_len < 2^32 here.
  */
@@ -177,6 +194,18 @@ GCM_API int gcm_decrypt_verify_host(gcm_ctx *ctx, const uint8_t iv[12],
                             const void *h_aad, uint64_t aad_len,
                             const void *h_ct, uint64_t len,
                             void *h_pt, const uint8_t tag[16], void *cuda_stream);
+
+/*
+ * Strict form of gcm_decrypt_verify_host: verify-then-release at the API level.  Pass 1
+ * streams the ciphertext through the GHASH-only kernel (no AES on the payload, nothing written to h_pt) and
+ * compares the tag on the device; only if it matches does pass 2 decrypt into h_pt.  No byte of unverified
+ * plaintext ever reaches the caller's buffer (on GCM_ERR_AUTH h_pt is left untouched), at the price of a second
+ * host-to-device transfer of the ciphertext.
+ */
+GCM_API int gcm_decrypt_verify_host_strict(gcm_ctx *ctx, const uint8_t iv[12],
+                                   const void *h_aad, uint64_t aad_len,
+                                   const void *h_ct, uint64_t len,
+                                   void *h_pt, const uint8_t tag[16], void *cuda_stream);
 
 /*
  * GHASH only (GMAC-style measurement; the paper's Table 5 "GHashKernelOnly",

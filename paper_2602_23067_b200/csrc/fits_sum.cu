@@ -82,14 +82,12 @@ uint32_t fits_sum_fold(unsigned long long s)
 extern "C" int gfc_datasum_async(const void *d_data, uint64_t len, void *d_acc, void *cuda_stream)
 {
     if (!d_acc || (len && !d_data) || ((uintptr_t)d_data & 15) || ((uintptr_t)d_acc & 7)) return GCM_ERR_ARG;
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return gcm_cuda_fail(e);
-    }
-    cudaError_t e = launch_fits_sum32((const uint8_t *)d_data, len, (unsigned long long *)d_acc, sms, (cudaStream_t)cuda_stream);
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);            // the data lives on the caller's current device
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    const int rc = gcm_sm_count(dev, &sms);        // cached per device
+    if (rc != GCM_OK) return rc;
+    e = launch_fits_sum32((const uint8_t *)d_data, len, (unsigned long long *)d_acc, sms, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? GCM_OK : gcm_cuda_fail(e);
 }
 

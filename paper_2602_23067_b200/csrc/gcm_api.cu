@@ -5,6 +5,8 @@
 #include <stdint.h>
 #include <string.h>
 #include <stdlib.h>
+#include <stddef.h>
+#include <atomic>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -15,8 +17,9 @@
 #include "gcm_fused.cuh"
 #include "gcm_api_internal.h"
 
-static int g_device = 0;
-static int g_last_cuda_error = 0;
+// Device for new contexts: -1 = the calling thread's current CUDA device, else the ordinal given to gcm_set_device.
+static std::atomic<int> g_device{-1};
+static std::atomic<int> g_last_cuda_error{0};
 
 // Wiped (device slab, pinned block) pairs of destroyed contexts, kept for the next gcm_init on the same
 // device: cudaMalloc + cudaHostAlloc cost milliseconds, the setup kernel 56 us (the paper pre-allocates
@@ -57,7 +60,7 @@ void pin_give(uint8_t *p)
 
 int gcm_cuda_fail(cudaError_t e)
 {
-    g_last_cuda_error = (int)e;
+    g_last_cuda_error.store((int)e);
     cudaGetLastError();   // clear the sticky-free error state
     return e == cudaErrorMemoryAllocation ? GCM_ERR_NOMEM : GCM_ERR_CUDA;
 }
@@ -68,19 +71,42 @@ int gcm_cuda_fail(cudaError_t e)
         if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
     } while (0)
 
-extern "C" const char *gcm_version(void) { return "b200gcm 0.1 sm_100a"; }
+extern "C" const char *gcm_version(void) { return "b200gcm 0.2 sm_100a"; }
 
 extern "C" int gcm_set_device(int ordinal)
 {
-    CU(cudaSetDevice(ordinal));
-    g_device = ordinal;
+    int count = 0;
+    CU(cudaGetDeviceCount(&count));
+    if (ordinal < -1 || ordinal >= count) return GCM_ERR_ARG;
+    g_device.store(ordinal);        // the caller's current device is left alone
     return GCM_OK;
 }
 
-extern "C" int gcm_last_cuda_error(void) { return g_last_cuda_error; }
+int gcm_default_device(int *device)
+{
+    const int d = g_device.load();
+    if (d >= 0) { *device = d; return GCM_OK; }
+    CU(cudaGetDevice(device));
+    return GCM_OK;
+}
+
+// SM count per device, queried once (cudaDeviceGetAttribute is cheap, but this sits on the latency path)
+int gcm_sm_count(int device, int *sms)
+{
+    static std::atomic<int> cache[GCM_MAX_DEVICES];
+    if (device >= 0 && device < GCM_MAX_DEVICES && cache[device].load(std::memory_order_relaxed) > 0) {
+        *sms = cache[device].load(std::memory_order_relaxed);
+        return GCM_OK;
+    }
+    CU(cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, device));
+    if (device >= 0 && device < GCM_MAX_DEVICES) cache[device].store(*sms, std::memory_order_relaxed);
+    return GCM_OK;
+}
+
+extern "C" int gcm_last_cuda_error(void) { return g_last_cuda_error.load(); }
 extern "C" const char *gcm_last_cuda_error_string(void)
 {
-    return cudaGetErrorString((cudaError_t)g_last_cuda_error);
+    return cudaGetErrorString((cudaError_t)g_last_cuda_error.load());
 }
 
 static void secure_zero(void *p, size_t n)      // memset the compiler may not drop
@@ -106,19 +132,30 @@ static SetupParams setup_params(gcm_ctx *c, const uint8_t *key)
 
 extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
 {
+    if (!out) return GCM_ERR_ARG;
+    *out = nullptr;
+    if (!key || (key_bits != 128 && key_bits != 256)) return GCM_ERR_ARG;     // before any CUDA call
+    int device = 0;
+    int rc = gcm_default_device(&device);
+    if (rc != GCM_OK) return rc;
+    return gcm_init_on_device(out, key, key_bits, device);
+}
+
+int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int device)
+{
     if (!out || !key || (key_bits != 128 && key_bits != 256)) return GCM_ERR_ARG;
     *out = nullptr;
-    CU(cudaSetDevice(g_device));
+    DeviceGuard guard(device);
+    CU(guard.err);
     // two attribute queries, not cudaGetDeviceProperties (which takes milliseconds)
     int sm_count = 0, smem_optin = 0;
-    CU(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, g_device));
-    CU(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, g_device));
+    CU(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device));
+    CU(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
     if ((size_t)smem_optin < (size_t)FUSED_SMEM_BYTES) return GCM_ERR_CUDA;
 
-    gcm_ctx *c = new (std::nothrow) gcm_ctx;
+    gcm_ctx *c = new (std::nothrow) gcm_ctx();      // value-initialised: every member zero
     if (!c) return GCM_ERR_NOMEM;
-    memset(c, 0, sizeof(*c));
-    c->device = g_device;
+    c->device = device;
     c->key_bits = key_bits;
     c->nr = key_bits == 128 ? 10 : 14;
     c->sm_count = sm_count;
@@ -137,7 +174,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
     {
         std::lock_guard<std::mutex> lock(g_pool_mu);
         for (size_t i = 0; i < g_pool.size(); i++)
-            if (g_pool[i].device == g_device && g_pool[i].bytes == c->slab_bytes) {
+            if (g_pool[i].device == device && g_pool[i].bytes == c->slab_bytes) {
                 c->d_slab = g_pool[i].d_slab;
                 g_pool.erase(g_pool.begin() + i);
                 break;
@@ -164,7 +201,10 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
         launch_setup(sp, 0);
         secure_zero(&sp, sizeof(sp));
         if ((e = cudaGetLastError()) != cudaSuccess) break;
-        if ((e = cudaMemcpy(c->h_rk, c->d_rk, sizeof(c->h_rk), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+        // synchronous copy: the tables are complete before any kernel of this context can be launched (the
+        // fused kernel reads them ahead of griddepcontrol.wait and relies on that)
+        static_assert(offsetof(gcm_ctx, h_rk) == offsetof(gcm_ctx, h_te0) + 1024, "h_te0 and h_rk are adjacent");
+        if ((e = cudaMemcpy(c->h_te0, c->d_te0, sizeof(c->h_te0) + sizeof(c->h_rk), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
     } while (0);
     if (e != cudaSuccess) {
         rc = gcm_cuda_fail(e);
@@ -178,7 +218,7 @@ extern "C" int gcm_init(gcm_ctx **out, const uint8_t *key, int key_bits)
 extern "C" void gcm_destroy(gcm_ctx *c)
 {
     if (!c) return;
-    cudaSetDevice(c->device);
+    DeviceGuard guard(c->device);
     gcm_host_pipe_free(c);
     bool pooled = false;
     if (c->d_slab) {
@@ -198,7 +238,7 @@ extern "C" void gcm_destroy(gcm_ctx *c)
     }
     if (!pooled && c->d_slab) cudaFree(c->d_slab);
     cudaGetLastError();
-    secure_zero(c, sizeof(*c));
+    secure_zero(c->h_rk, sizeof(c->h_rk));
     delete c;
 }
 
@@ -206,7 +246,7 @@ void gcm_pool_release(void)
 {
     std::lock_guard<std::mutex> lock(g_pool_mu);
     for (const PooledSlab &p : g_pool) {           // already wiped when they were pooled
-        cudaSetDevice(p.device);
+        DeviceGuard guard(p.device);
         cudaFree(p.d_slab);
     }
     g_pool.clear();
@@ -240,15 +280,23 @@ extern "C" int gcm_get_geometry(const gcm_ctx *c, int *grid, int *threads)
 extern "C" int gcm_get_hash_subkey(const gcm_ctx *c, uint8_t h[16])
 {
     if (!c || !h) return GCM_ERR_ARG;
-    CU(cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    CU(guard.err);
     CU(cudaMemcpy(h, c->d_h, 16, cudaMemcpyDeviceToHost));
     return GCM_OK;
 }
 
-// Argument checks and launch parameters common to encrypt / decrypt / ghash.  ctr_base: index of
-// the first payload block of this launch within its message (0 except in the chunked host pipeline).
+extern "C" int gcm_set_phase_stamps(gcm_ctx *c, void *d_stamps)
+{
+    if (!c) return GCM_ERR_ARG;
+    c->d_stamps = (unsigned long long *)d_stamps;
+    return GCM_OK;
+}
+
+// Argument checks and launch parameters common to encrypt / decrypt / ghash (see gcm_api_internal.h).
 int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad, uint64_t aad_len,
-                     const void *d_in, uint64_t len, void *d_out, uint32_t ctr_base, GcmParams *p, int *blocks)
+                     const void *d_in, uint64_t len, void *d_out, uint32_t ctr_base, bool last,
+                     uint64_t final_len, uint64_t final_aad_len, GcmParams *p, int *blocks)
 {
     if (!c) return GCM_ERR_ARG;
     if (mode != MODE_GHASH && !iv) return GCM_ERR_ARG;
@@ -257,42 +305,24 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     if (mode != MODE_GHASH && len && !d_out) return GCM_ERR_ARG;
     const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
     if (mode != MODE_GHASH && len && a != b && a < b + len && b < a + len) return GCM_ERR_ARG;  // partial overlap
+    if ((aad_len + 15) / 16 > 0xFFFFFFFFull) return GCM_ERR_LEN;
 
     memset(p, 0, sizeof(*p));
+    row_msg_fill(p->m, (const uint8_t *)d_in, (uint8_t *)d_out, (const uint8_t *)d_aad, len, aad_len, ctr_base,
+                 last ? 1u : 0u, final_len, final_aad_len, mode == MODE_GHASH);
+    if (p->m.vblocks >= GCM_MAX_VBLOCKS) return GCM_ERR_LEN;
     memcpy(p->rk, c->h_rk, sizeof(p->rk));
+    memcpy(p->te0, c->h_te0, sizeof(p->te0));
     if (iv) memcpy(p->iv, iv, 12);
-    p->in = (const uint8_t *)d_in;
-    p->out = (uint8_t *)d_out;
-    p->aad = (const uint8_t *)d_aad;
-    p->len = len;
-    p->aad_len = aad_len;
-    p->final_len = len;
-    p->final_aad_len = aad_len;
-    const uint64_t n_full = len / 16, n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
-    if (n_aad > 0xFFFFFFFFull) return GCM_ERR_LEN;
-    // leading zero blocks (free in GHASH) make counter == virtual index (mod 32)
-    const uint32_t pad = (2u + ctr_base - (uint32_t)n_aad) & (GCM_STRIDE - 1);
-    const uint64_t base = (uint64_t)pad + n_aad;
-    const uint64_t E = base + n_blocks;
-    if (E >= GCM_MAX_VBLOCKS) return GCM_ERR_LEN;
-    const uint64_t S = (E + GCM_STRIDE - 1) / GCM_STRIDE;
+    // rows are dealt to the warps of the grid in contiguous runs balanced to +-1 row; a short message uses
+    // only as many CTAs as it has rows for
+    const uint64_t S = p->m.rows;
     const uint64_t wpc = (uint64_t)c->threads / 32;              // warps per CTA
-    const uint64_t W = (uint64_t)c->grid * wpc;
-    uint64_t Q = (S + W - 1) / W;
-    if (Q < 1) Q = 1;
-    p->pad = pad;
-    p->n_aad_blocks = (uint32_t)n_aad;
-    p->base = base;
-    p->vblocks = E;
-    p->rows = (uint32_t)S;
-    p->rows_per_warp = (uint32_t)Q;
-    p->ctr_delta = ctr_base + 2u - (uint32_t)base;
-    p->aligned = (((a | (mode == MODE_GHASH ? 0 : b)) & 15) == 0) ? 1u : 0u;
-    if (p->aligned) {
-        p->fast_lo = (uint32_t)((base + GCM_STRIDE - 1) / GCM_STRIDE);
-        p->fast_hi = (uint32_t)((base + n_full) / GCM_STRIDE);
-        if (p->fast_hi < p->fast_lo) p->fast_hi = p->fast_lo;
-    }
+    uint64_t want = (S + wpc - 1) / wpc;
+    if (want < 1) want = 1;
+    if (want > (uint64_t)c->grid) want = (uint64_t)c->grid;
+    *blocks = (int)want;
+    p->warps = (uint32_t)(want * wpc);
     p->tab.te0 = c->d_te0;
     p->tab.ktab = c->d_ktab;
     p->tab.hpow = c->d_hpow;
@@ -300,54 +330,76 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     p->tab.h = c->d_h;
     p->partials = c->d_partials;
     p->counter = c->d_counter;
+    c->ticket_next += (unsigned)want;                            // epoch scheme: see GcmParams::ticket_last
+    p->ticket_last = c->ticket_next - 1;
     p->tag_out = c->d_tag;
     p->status = c->d_status;
-    const uint64_t active_warps = (S + Q - 1) / Q;
-    uint64_t want = (active_warps + wpc - 1) / wpc;
-    if (want < 1) want = 1;
-    *blocks = (int)want;
+    p->stamps = c->d_stamps;
     return GCM_OK;
 }
 
 // Header-sized messages take the single-CTA latency kernel (gcm_small.cu) under the default geometry; an
 // explicit gcm_set_geometry always selects the fused kernel (the geometry tests rely on that).
-static cudaError_t launch_auto(gcm_ctx *c, int mode, int blocks, const GcmParams &p, cudaStream_t s)
+cudaError_t gcm_launch_fused(gcm_ctx *c, int mode, int blocks, const GcmParams &p, cudaStream_t s)
 {
-    const uint64_t n_ghash = (uint64_t)p.n_aad_blocks + (p.len + 15) / 16 + 1;
-    if (mode != MODE_GHASH && n_ghash <= SMALL_MAX_BLOCKS && c->grid == c->sm_count && c->threads == GCM_MAX_THREADS &&
-        !p.chain_in && !p.chain_out)
-        return launch_small(c->nr, mode, p, s);
-    return launch_fused(c->nr, mode, c->threads, blocks, p, s);
+    const cudaError_t e = launch_fused(c->nr, mode, c->threads, blocks, p, s);
+    if (e != cudaSuccess) c->ticket_next -= (unsigned)blocks;    // the launch was not made: its tickets are not drawn
+    return e;
 }
 
-extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
-                                 const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
+static cudaError_t launch_auto(gcm_ctx *c, int mode, int blocks, GcmParams &p, cudaStream_t s)
+{
+    const uint64_t n_ghash = (uint64_t)p.m.n_aad_blocks + (p.m.len + 15) / 16 + 1;
+    if (mode != MODE_GHASH && n_ghash <= SMALL_MAX_BLOCKS && c->grid == c->sm_count && c->threads == GCM_MAX_THREADS &&
+        !p.chain_in && !p.chain_out) {
+        c->ticket_next -= (unsigned)blocks;                      // no tickets are drawn by the latency kernel
+        return launch_small(c->nr, mode, p, s);
+    }
+    return gcm_launch_fused(c, mode, blocks, p, s);
+}
+
+#define LOCK_CTX(c)                                                                                \
+    if (!(c)) return GCM_ERR_ARG;                                                                  \
+    CtxLock lock__(c);                                                                             \
+    if (!lock__.ok) return GCM_ERR_BUSY;                                                           \
+    DeviceGuard guard__((c)->device);                                                              \
+    CU(guard__.err)
+
+static int encrypt_async_locked(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                                const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
 {
     GcmParams p;
     int blocks = 0;
     if (!d_tag) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, 0, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_tag;
-    CU(cudaSetDevice(c->device));
     cudaError_t e = launch_auto(c, MODE_ENCRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;
 }
 
+extern "C" int gcm_encrypt_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
+                                 const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
+{
+    LOCK_CTX(c);
+    return encrypt_async_locked(c, iv, d_aad, aad_len, d_pt, len, d_ct, d_tag, stream);
+}
+
 extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
                                         const void *d_ct, uint64_t len, void *d_pt, const void *d_tag,
                                         void *d_status, void *stream)
 {
+    LOCK_CTX(c);
     GcmParams p;
     int blocks = 0;
     if (!d_tag || !d_status) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_in = (const uint4 *)d_tag;
     p.status = (int *)d_status;
-    CU(cudaSetDevice(c->device));
+    p.status_init = 1;          // the verdict word reads "refused" until the finisher has written it (fail closed)
     cudaError_t e = launch_auto(c, MODE_DECRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
@@ -360,14 +412,14 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
 extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, const void *d_c, uint64_t len,
                                void *d_out, void *stream)
 {
+    LOCK_CTX(c);
     GcmParams p;
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
-    int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_out;
-    CU(cudaSetDevice(c->device));
-    cudaError_t e = launch_fused(c->nr, MODE_GHASH, c->threads, blocks, p, (cudaStream_t)stream);
+    cudaError_t e = gcm_launch_fused(c, MODE_GHASH, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;
@@ -376,10 +428,11 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
 extern "C" int gcm_encrypt(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
                            const void *d_pt, uint64_t len, void *d_ct, uint8_t tag[16], void *stream)
 {
-    if (!c || !tag) return GCM_ERR_ARG;
+    if (!tag) return GCM_ERR_ARG;
+    LOCK_CTX(c);
     // the finishing thread stores the tag straight into mapped pinned host memory (unified addressing):
     // one posted PCIe write instead of a separate D2H copy on the latency path
-    int rc = gcm_encrypt_async(c, iv, d_aad, aad_len, d_pt, len, d_ct, c->h_pinned, stream);
+    int rc = encrypt_async_locked(c, iv, d_aad, aad_len, d_pt, len, d_ct, c->h_pinned, stream);
     if (rc != GCM_OK) return rc;
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     memcpy(tag, c->h_pinned, 16);
@@ -389,21 +442,23 @@ extern "C" int gcm_encrypt(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, 
 extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
                                   const void *d_ct, uint64_t len, void *d_pt, const uint8_t tag[16], void *stream)
 {
-    if (!c || !tag) return GCM_ERR_ARG;
+    if (!tag) return GCM_ERR_ARG;
+    LOCK_CTX(c);
     GcmParams p;
     int blocks = 0;
-    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, &p, &blocks);
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
-    p.status = (int *)(c->h_pinned + 16);   // verdict written straight into mapped pinned host memory
-    CU(cudaSetDevice(c->device));
+    // verdict written straight into mapped pinned host memory; it reads "refused" until the finisher says
+    // otherwise, so a launch that never finishes cannot pass for an accepted message (fail closed)
+    volatile int *verdict = (volatile int *)(c->h_pinned + 16);
+    *verdict = GCM_STATUS_PENDING;
+    p.status = (int *)(c->h_pinned + 16);
     cudaError_t e = launch_auto(c, MODE_DECRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     CU(cudaStreamSynchronize((cudaStream_t)stream));
-    int status;
-    memcpy(&status, c->h_pinned + 16, 4);
-    if (status != 0) {
+    if (*verdict != 0) {
         launch_wipe((uint8_t *)d_pt, len, nullptr, (cudaStream_t)stream);
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize((cudaStream_t)stream));

@@ -15,9 +15,9 @@
 //   a10-a11  length block, tag, constant-time compare, zero-fill of the output on mismatch.
 // Keys never touch global memory except inside the descriptor array, which is wiped after the call.
 //
-// Large messages (FITS-sized HDUs, config C3) go through the fused single-message kernel with a
-// per-key context that is cached across calls, one asynchronous launch per message on the caller's
-// stream; tags and verdicts of both paths come back in one copy.
+// Large messages (>= BATCH_LARGE_BYTES: FITS-sized HDUs, config C3) are grouped by key and go through
+// gcm_multi_kernel (gcm_multi.cu), ONE launch per key with a per-key context that is cached across calls; tags and
+// verdicts of both paths come back in one copy.
 #include <cuda_runtime.h>
 #include <string.h>
 #include <algorithm>
@@ -32,6 +32,7 @@
 #include "gcm_device.cuh"
 #include "gcm_setup.cuh"
 #include "gcm_multi.cuh"
+#include "gcm_fused.cuh"
 #include "gcm_api_internal.h"
 
 #define BATCH_WARPS        12
@@ -83,6 +84,22 @@ __device__ __forceinline__ uint4 ghash_mul4(const uint8_t *tab, const uint32_t (
     return acc;
 }
 
+struct MulK4 {                 // the warp's own 4-bit Shoup table of K (row loop multiplier)
+    const uint8_t *tab;
+    uint32_t rot[8], col[8];
+    __device__ __forceinline__ MulK4(const uint8_t *tab_, uint32_t lane) : tab(tab_)
+    {
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            const uint32_t n = (lane + k) & 7;
+            const uint32_t sh = 8 * (n >> 1) + ((n & 1) ? 0 : 4);    // bit position of the nibble in its word
+            rot[k] = (sh - 9) & 31;
+            col[k] = n * 16;
+        }
+    }
+    __device__ __forceinline__ uint4 operator()(uint4 y) const { return ghash_mul4(tab, rot, col, y); }
+};
+
 __device__ __forceinline__ uint4 shfl4(uint4 v, uint32_t src)
 {
     return make_uint4(__shfl_sync(0xFFFFFFFFu, v.x, src), __shfl_sync(0xFFFFFFFFu, v.y, src),
@@ -127,75 +144,14 @@ __device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *r
     }
     __syncwarp();
 
-    uint32_t rot[8], col[8];
-#pragma unroll
-    for (int k = 0; k < 8; k++) {
-        const uint32_t n = (lane + k) & 7;
-        const uint32_t sh = 8 * (n >> 1) + ((n & 1) ? 0 : 4);    // bit position of the nibble in its word
-        rot[k] = (sh - 9) & 31;
-        col[k] = n * 16;
-    }
-
-    // the virtual block sequence [pad | AAD | payload] of the fused kernel, all rows in this warp
-    const uint64_t len = d.len, aad_len = d.aad_len;
-    const uint64_t n_full = len / 16, n_blocks = (len + 15) / 16, n_aad = (aad_len + 15) / 16;
-    const uint32_t pad = (2u - (uint32_t)n_aad) & 31;
-    const uint64_t base = pad + n_aad, E = base + n_blocks;
-    const uint32_t S = (uint32_t)((E + 31) / 32);
-    const uint32_t ctr_delta = 2u - (uint32_t)base;
-    const bool aligned = ((((uintptr_t)d.in) | ((uintptr_t)d.out)) & 15) == 0;
-    uint32_t fast_lo = 0, fast_hi = 0;
-    if (aligned) {
-        fast_lo = (uint32_t)((base + 31) / 32);
-        fast_hi = (uint32_t)((base + n_full) / 32);
-        if (fast_hi < fast_lo) fast_hi = fast_lo;
-    }
-
+    // the virtual block sequence [pad | AAD | payload | length block] of the fused kernel, all rows in this warp
+    RegMsgView m;
+    row_msg_fill(m.r, d.in, d.out, d.aad, d.len, d.aad_len, 0u, 1u, d.len, d.aad_len, false);
+    const uint64_t E = m.r.vblocks;
+    const uint32_t S = m.r.rows;
+    const MulK4 mul(tab, lane);
     const CtrConst cc = ctr_const(rk, d.iv[0], d.iv[1], d.iv[2], sm, lane4);
-    CtrCache cu = {0, 0, 0, 0};
-    uint4 Y = make_uint4(0, 0, 0, 0), pre = make_uint4(0, 0, 0, 0);
-    bool have_pre = false;
-#pragma unroll 1
-    for (uint32_t row = 0; row < S; row++) {
-        const uint64_t v = 32ull * row + lane;
-        const bool fast = row >= fast_lo && row < fast_hi;
-        uint4 x = make_uint4(0, 0, 0, 0);
-        uint32_t cbytes = 0;
-        uint64_t g = 0;
-        bool valid = true;
-        if (fast) {
-            g = v - base;
-            x = have_pre ? pre : ld16_stream(d.in + 16 * g);
-            cbytes = 16;
-            have_pre = row + 1 < fast_hi;
-            if (have_pre) pre = ld16_stream(d.in + 16 * g + 512);
-        } else {
-            have_pre = false;
-            valid = v < E;
-            if (valid && v >= pad) {
-                const uint64_t u = v - pad;
-                if (u < n_aad) {
-                    const uint64_t rem = aad_len - 16 * u;
-                    x = load_bytes(d.aad + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
-                } else {
-                    g = u - n_aad;
-                    const uint64_t rem = len - 16 * g;
-                    cbytes = rem < 16 ? (uint32_t)rem : 16u;
-                    x = (cbytes == 16 && aligned) ? ld16_stream(d.in + 16 * g) : load_bytes(d.in + 16 * g, cbytes);
-                }
-            }
-        }
-        const uint4 ym = ghash_mul4(tab, rot, col, Y);           // a7
-        const uint32_t ctr = (uint32_t)v + ctr_delta;            // a4
-        if (row == 0 || (ctr & 0xE0u) == 0) cu = ctr_cache(rk, sm, lane4, cc, ctr);
-        const uint4 ks = aes_ctr_block<NR>(rk, sm, lane4, cc, cu, ctr);   // a5
-        const uint4 y = xor4(x, ks);                             // a6
-        if (cbytes == 16 && (fast || aligned)) st16_stream(d.out + 16 * g, y);
-        else if (cbytes) store_bytes(d.out + 16 * g, y, cbytes);
-        uint4 X = x;
-        if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
-        if (fast || valid) Y = xor4(ym, X);
-    }
+    const uint4 Y = gcm_rows<NR, MODE>(m, rk, sm, lane, cc, 0u, S, mul);        // a4-a7 (a10: the length block is a row block)
 
     // a8: the tree over the lanes, in the order of their last blocks (rotate by the ragged remainder):
     // index i = (lane - rem) & 31 holds the partial whose last block is 31 - i blocks before the end.
@@ -209,13 +165,9 @@ __device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *r
         const uint4 prod = gf_mul_mem(left, hp[k]);
         if ((i & ((2u << k) - 1)) == (2u << k) - 1) Z = xor4(Z, prod);
     }
-    // index 31 (lane (31 + rem) & 31) now holds sum X_v . H^(E - 1 - v); a10: one H for the chain, then
-    // the length block and the last H
-    const uint64_t abits = aad_len * 8, cbits = len * 8;
-    const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
-                               bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
-    const uint4 acc = gf_mul_mem(Z, h);
-    const uint4 Sg = gf_mul_mem(xor4(acc, L), h);
+    // index 31 (lane (31 + rem) & 31) now holds sum X_v . H^(E - 1 - v) with the length block as the last X_v:
+    // one more H gives GHASH_H(A, C)
+    const uint4 Sg = gf_mul_mem(Z, h);
     const uint4 tag = shfl4(xor4(Sg, ekj0), (31 + rem) & 31);    // a11
     if (MODE == MODE_ENCRYPT) {
         if (lane == 0) {
@@ -227,6 +179,7 @@ __device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *r
         if (lane == 0) res->status = diff != 0 ? 1 : 0;
         if (diff != 0) {                                        // payload suppression
             __syncwarp();
+            const uint64_t len = d.len;
             uint64_t head = (16 - ((uintptr_t)d.out & 15)) & 15;
             if (head > len) head = len;
             const uint64_t mid = (len - head) / 16;
@@ -247,7 +200,7 @@ gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *o
     extern __shared__ __align__(1024) uint8_t sm[];
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t warp = __shfl_sync(0xFFFFFFFFu, threadIdx.x >> 5, 0);
-    fill_aes_tables<BATCH_THREADS>(sm, te0);
+    fill_aes_tables<BATCH_THREADS>(sm, te0, threadIdx.x);
     __syncthreads();
     uint8_t *tab = sm + BATCH_TAB_OFF + warp * BATCH_TAB_BYTES;
     uint4 *hp = reinterpret_cast<uint4 *>(sm + BATCH_HP_OFF + warp * BATCH_HP_BYTES);
@@ -267,8 +220,9 @@ template <int NR, int MODE>
 static cudaError_t launch_batch(int blocks, const BatchDesc *descs, BatchResult *results, const uint32_t *order,
                                 uint32_t n, unsigned *next, const uint32_t *te0, cudaStream_t s)
 {
+    static std::atomic<bool> configured[GCM_MAX_DEVICES];
     auto kern = gcm_batch_kernel<NR, MODE>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, BATCH_SMEM_BYTES);
+    cudaError_t e = ensure_smem_attr((const void *)kern, configured, BATCH_SMEM_BYTES);
     if (e != cudaSuccess) return e;
     kern<<<blocks, BATCH_THREADS, BATCH_SMEM_BYTES, s>>>(descs, results, order, n, next, te0);
     return cudaGetLastError();
@@ -309,7 +263,7 @@ void secure_zero(void *p, size_t n)
 void free_staging_locked()
 {
     if (g.device < 0) return;
-    cudaSetDevice(g.device);
+    DeviceGuard guard(g.device);
     if (g.d_desc) { launch_wipe((uint8_t *)g.d_desc, (uint64_t)g.cap * sizeof(BatchDesc), nullptr, 0); cudaDeviceSynchronize(); cudaFree(g.d_desc); }
     if (g.h_desc) { secure_zero(g.h_desc, (size_t)g.cap * sizeof(BatchDesc)); cudaFreeHost(g.h_desc); }
     if (g.d_res) cudaFree(g.d_res);
@@ -336,9 +290,11 @@ void evict_keys_locked()
 
 int ensure_staging_locked(uint32_t n)
 {
+    // one notion of "the device" for the whole library: gcm_set_device's choice, else the caller's current device
     int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    int rc0 = gcm_default_device(&dev);
+    if (rc0 != GCM_OK) return rc0;
+    cudaError_t e = cudaSuccess;
     if (g.device != dev || g.cap < n) {
         free_staging_locked();
         cudaDeviceProp prop;
@@ -379,7 +335,7 @@ int ctx_for_key_locked(const uint8_t *key, int key_bits, gcm_ctx **out)
     auto it = g.by_key.find(id);
     if (it != g.by_key.end()) { *out = it->second; secure_zero(&id[0], id.size()); return GCM_OK; }
     gcm_ctx *c = nullptr;
-    int rc = gcm_init(&c, key, key_bits);
+    int rc = gcm_init_on_device(&c, key, key_bits, g.device);
     if (rc == GCM_OK) { g.by_key[id] = c; *out = c; }
     secure_zero(&id[0], id.size());
     return rc;
@@ -458,24 +414,11 @@ int run_large_locked(gcm_msg *msgs, const std::vector<uint32_t> &large, bool dec
             const gcm_msg &m = msgs[idx[j]];
             MultiMsg &d = mm[j];
             memcpy(d.iv, m.iv, 12);
-            const uint64_t n_full = m.len / 16, n_blocks = (m.len + 15) / 16, n_aad = (m.aad_len + 15) / 16;
-            d.pad = (2u - (uint32_t)n_aad) & (GCM_STRIDE - 1);
-            d.in = (const uint8_t *)m.d_in; d.out = (uint8_t *)m.d_out; d.aad = (const uint8_t *)m.d_aad;
-            d.len = m.len; d.aad_len = m.aad_len;
-            d.base = (uint64_t)d.pad + n_aad;
-            d.vblocks = d.base + n_blocks;
-            d.n_aad_blocks = (uint32_t)n_aad;
-            d.rows = (uint32_t)((d.vblocks + GCM_STRIDE - 1) / GCM_STRIDE);
-            d.aligned = ((((uintptr_t)m.d_in) | ((uintptr_t)m.d_out)) & 15) == 0 ? 1u : 0u;
-            if (d.aligned) {
-                d.fast_lo = (uint32_t)((d.base + GCM_STRIDE - 1) / GCM_STRIDE);
-                d.fast_hi = (uint32_t)((d.base + n_full) / GCM_STRIDE);
-                if (d.fast_hi < d.fast_lo) d.fast_hi = d.fast_lo;
-            }
-            d.ctr_delta = 2u - (uint32_t)d.base;
+            row_msg_fill(d.m, (const uint8_t *)m.d_in, (uint8_t *)m.d_out, (const uint8_t *)m.d_aad, m.len, m.aad_len,
+                         0u, 1u, m.len, m.aad_len, false);
             if (decrypt) memcpy(d.tag_expect, m.tag, 16);
             d.result = idx[j];
-            R += d.rows;
+            R += d.m.rows;
         }
         const uint64_t Q = std::max<uint64_t>(1, (R + W - 1) / W);
         uint32_t w = 0, nch = 0;
@@ -483,8 +426,8 @@ int run_large_locked(gcm_msg *msgs, const std::vector<uint32_t> &large, bool dec
         wf[0] = 0;
         for (size_t j = 0; j < idx.size(); j++) {
             uint32_t r = 0;
-            while (r < mm[j].rows) {
-                const uint32_t take = (uint32_t)std::min<uint64_t>(budget, mm[j].rows - r);
+            while (r < mm[j].m.rows) {
+                const uint32_t take = (uint32_t)std::min<uint64_t>(budget, mm[j].m.rows - r);
                 ch[nch].msg = (uint32_t)j; ch[nch].r0 = r; ch[nch].r1 = r + take;
                 nch++; r += take; budget -= take;
                 if (budget == 0) { wf[++w] = nch; budget = Q; }
@@ -497,6 +440,7 @@ int run_large_locked(gcm_msg *msgs, const std::vector<uint32_t> &large, bool dec
         memset(&p, 0, sizeof(p));
         gcm_ctx *c = groups[k].ctx;
         memcpy(p.rk, c->h_rk, sizeof(p.rk));
+        memcpy(p.te0, c->h_te0, sizeof(p.te0));
         p.tab.te0 = c->d_te0; p.tab.ktab = c->d_ktab; p.tab.hpow = c->d_hpow; p.tab.hx = c->d_hx; p.tab.h = c->d_h;
         p.msgs = (const MultiMsg *)(g.d_multi + lay[k].msgs);
         p.chunks = (const MultiChunk *)(g.d_multi + lay[k].chunks);
@@ -528,7 +472,12 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     if (n == 0) return GCM_OK;
     std::lock_guard<std::mutex> lock(g.mu);
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = ensure_staging_locked(n);
+    int dev = 0;
+    int rc = gcm_default_device(&dev);
+    if (rc != GCM_OK) return rc;
+    DeviceGuard guard(dev);                                 // staging, per-key contexts and kernels all live on `dev`
+    CUB(guard.err);
+    rc = ensure_staging_locked(n);
     if (rc != GCM_OK) return rc;
 
     int first_err = GCM_OK;

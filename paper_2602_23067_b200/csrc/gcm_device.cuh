@@ -232,53 +232,245 @@ __device__ __forceinline__ uint4 cta_xor_reduce(uint4 v, uint4 *red)
     return v;
 }
 
-// Table fill at kernel start, latency-critical for small messages (header-sized messages): all
-// global loads of a thread are issued before its first shared-memory store, so the fill costs about one L2
-// round trip plus the 1536 store wavefronts of the 192 KB, instead of one round trip per loop iteration.
-template <int TPB>
-__device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const uint32_t *te0)
+// AES table fill at kernel start, latency-critical for small and FITS-sized messages (Table A.7):
+// the 1 KB round table T0 travels in the kernel parameter block (constant bank), so the expansion into the 128 KB
+// lane-replicated layout needs no global load at all: one warp-uniform constant read and two 16-byte stores per
+// four table words, 1024 store wavefronts per CTA in total.  Threads tid = 0 .. NT-1 share the work.
+template <int NT, class TE0>
+__device__ __forceinline__ void fill_aes_tables(uint8_t *sm, const TE0 &te0, uint32_t tid)
 {
-    uint32_t *a0 = reinterpret_cast<uint32_t *>(sm + AES_A0_OFF);
-    uint32_t *a1 = reinterpret_cast<uint32_t *>(sm + AES_A1_OFF);
-    constexpr int ROWS = (256 * 64 + TPB - 1) / TPB;       // table words per thread and array
-    uint32_t te[ROWS];
-#pragma unroll
-    for (int k = 0; k < ROWS; k++) {
-        const uint32_t j = threadIdx.x + k * TPB;
-        te[k] = j < 16384 ? __ldg(te0 + (j >> 6)) : 0u;
+    uint4 *a0 = reinterpret_cast<uint4 *>(sm + AES_A0_OFF);
+    uint4 *a1 = reinterpret_cast<uint4 *>(sm + AES_A1_OFF);
+    // group g = four consecutive words of one 256-byte row (64 words: 32 x T_even | 32 x T_odd): 16 groups per row
+#pragma unroll 4
+    for (uint32_t g = tid; g < 4096; g += NT) {
+        const uint32_t te = te0[g >> 4];
+        const bool odd = (g >> 3) & 1;
+        const uint32_t v0 = odd ? rotl32(te, 8) : te;                   // T0 | T1
+        const uint32_t v1 = odd ? rotl32(te, 24) : rotl32(te, 16);      // T2 | T3
+        a0[g] = make_uint4(v0, v0, v0, v0);
+        a1[g] = make_uint4(v1, v1, v1, v1);
     }
-#pragma unroll
-    for (int k = 0; k < ROWS; k++) {
-        const uint32_t j = threadIdx.x + k * TPB;
-        if (j < 16384) {
-            const bool odd = (j >> 5) & 1;
-            a0[j] = odd ? rotl32(te[k], 8) : te[k];                 // T0 | T1
-            a1[j] = odd ? rotl32(te[k], 24) : rotl32(te[k], 16);    // T2 | T3
+}
+
+// ---- sm_100a plumbing: bulk copy (TMA 1-D) completing on an mbarrier, programmatic dependent launch ----------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");      // visible to the async proxy
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completes on `bar` (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_copy_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// Programmatic dependent launch: the next kernel of the stream may start its prologue (table fill) while this
+// grid drains; it must not touch stream-ordered data before pdl_wait().  Both are no-ops for a plain launch.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// Shared-memory tables at kernel start.  The 64 KB GHASH multiplier table comes straight from the context slab by
+// ONE bulk copy (TMA 1-D: cp.async.bulk, SASS UBLKCP) issued by thread 0 and completing on an mbarrier: no register
+// staging, no store wavefronts; meanwhile the other threads expand the round table (above).  Reading the AES tables
+// pre-expanded from L2 instead would move 128 KB per CTA x 148 CTAs = 19 MB through L2 per launch (2 us at the
+// measured L2 rate) where the expansion costs 0.5 us of stores and no memory traffic.  With SPARE_WARP0 the first
+// warp takes no part in the expansion (it has the position weights to form).  Call tables_wait() before the first
+// table read.
+template <int TPB, bool WITH_AES, bool SPARE_WARP0, class TE0>
+__device__ __forceinline__ void tables_begin(uint8_t *sm, const GcmTables &tab, const TE0 &te0)
+{
+    uint64_t *bar = reinterpret_cast<uint64_t *>(sm + MBAR_OFF);
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, KTAB_BYTES);
+        bulk_copy_g2s(sm + KTAB_OFF, tab.ktab, KTAB_BYTES, bar);
+    }
+    if (WITH_AES) {
+        if (SPARE_WARP0 && TPB > 32) {
+            if (threadIdx.x >= 32) fill_aes_tables<TPB - 32>(sm, te0, threadIdx.x - 32);
+        } else {
+            fill_aes_tables<TPB>(sm, te0, threadIdx.x);
         }
     }
 }
-
-// The GHASH multiplier table: global loads into registers first (ktab_load), stores after the AES tables
-// have been written (ktab_store), so the two fills share one memory round trip.
-template <int TPB>
-struct KtabRegs { uint4 v[(KTAB_BYTES / 16 + TPB - 1) / TPB]; };
-
-template <int TPB>
-__device__ __forceinline__ void ktab_load(KtabRegs<TPB> &r, const uint4 *ktab)
+__device__ __forceinline__ void tables_wait(uint8_t *sm)
 {
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(r.v) / sizeof(uint4)); k++) {
-        const uint32_t j = threadIdx.x + k * TPB;
-        r.v[k] = j < KTAB_BYTES / 16 ? __ldg(ktab + j) : make_uint4(0, 0, 0, 0);
-    }
+    __syncthreads();                                       // AES tables stored, mbarrier initialised
+    mbar_wait(reinterpret_cast<uint64_t *>(sm + MBAR_OFF), 0);
 }
-template <int TPB>
-__device__ __forceinline__ void ktab_store(const KtabRegs<TPB> &r, uint8_t *sm)
+
+// ---- GHASH multipliers for the row loop -----------------------------------------------------------------------
+struct MulK8 {                 // 8-bit Shoup table of K in shared memory at KTAB_OFF (fused / multi kernels)
+    const uint8_t *sm;
+    uint32_t sel[8];
+    __device__ __forceinline__ MulK8(const uint8_t *sm_, uint32_t lane) : sm(sm_)
+    {
+#pragma unroll
+        for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
+    }
+    __device__ __forceinline__ uint4 operator()(uint4 y) const { return ghash_mul_k(sm, sel, y); }
+};
+
+// ---- the row loop: SURVEY.md 8(a) a4-a7 for rows [r0, r1) of one message ------------------------------------
+// MSG: accessor view of a RowMsg (hot fields in registers or constant bank, cold ones wherever they live).
+// RK:  indexable round keys.  MUL: y -> y . K.  Returns the lane's running value Y (a7) after its last block.
+// The same code serves the single-message kernel (gcm_fused.cu), the many-large-messages kernel (gcm_multi.cu)
+// and the warp-per-message kernel (gcm_batch.cu).
+template <int NR, int MODE, class MSG, class RK, class MUL>
+__device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint8_t *sm, uint32_t lane,
+                                          const CtrConst &cc, uint32_t r0, uint32_t r1, const MUL &mul)
 {
-    uint4 *kt = reinterpret_cast<uint4 *>(sm + KTAB_OFF);
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(r.v) / sizeof(uint4)); k++) {
-        const uint32_t j = threadIdx.x + k * TPB;
-        if (j < KTAB_BYTES / 16) kt[j] = r.v[k];
+    const uint32_t lane4 = lane * 4;
+    CtrCache cu = {0, 0, 0, 0};
+    uint4 Y = make_uint4(0, 0, 0, 0);
+    uint4 pre = make_uint4(0, 0, 0, 0);
+    bool have_pre = false;
+    for (uint32_t row = r0; row < r1; row++) {
+        const uint64_t v = 32ull * row + lane;          // virtual block index
+        const bool fast = row >= m.fast_lo() && row < m.fast_hi();
+        uint4 x = make_uint4(0, 0, 0, 0);
+        uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD / length block / beyond the end)
+        uint64_t g = 0;                                 // payload block index
+        bool valid = true;
+        if (fast) {
+            g = v - m.base();
+            x = have_pre ? pre : ld16_stream(m.in() + 16 * g);
+            cbytes = 16;
+            have_pre = row + 1 < r1 && row + 1 < m.fast_hi();
+            if (have_pre) pre = ld16_stream(m.in() + 16 * g + 512);
+        } else {
+            have_pre = false;
+            valid = v < m.vblocks();
+            if (valid && v >= m.pad()) {
+                const uint64_t u = v - m.pad();
+                if (u < m.n_aad_blocks()) {
+                    const uint64_t rem = m.aad_len() - 16 * u;
+                    x = load_bytes(m.aad() + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
+                } else if (m.len_block() && v + 1 == m.vblocks()) {      // a10: BE64(8 a) || BE64(8 len)
+                    const uint64_t abits = m.final_aad_len() * 8, cbits = m.final_len() * 8;
+                    x = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
+                                   bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
+                } else {
+                    g = u - m.n_aad_blocks();
+                    const uint64_t rem = m.len() - 16 * g;
+                    cbytes = rem < 16 ? (uint32_t)rem : 16u;
+                    x = (cbytes == 16 && m.aligned()) ? ld16_stream(m.in() + 16 * g) : load_bytes(m.in() + 16 * g, cbytes);
+                }
+            }
+        }
+        // a7: multiply the running value by K; independent of this row's AES, so they interleave
+        const uint4 ym = mul(Y);
+        uint4 X = x;
+        if (MODE != MODE_GHASH) {
+            // a4: counter from the virtual index alone; the upper 24 bits are warp-uniform and change
+            // every 8th row, when rounds 1-2 are re-cached
+            const uint32_t ctr = (uint32_t)v + m.ctr_delta();
+            if (row == r0 || (ctr & 0xE0u) == 0) cu = ctr_cache(rk, sm, lane4, cc, ctr);
+            const uint4 ks = aes_ctr_block<NR>(rk, sm, lane4, cc, cu, ctr);     // a5
+            const uint4 y = xor4(x, ks);                                   // a6
+            if (cbytes == 16 && (fast || m.aligned())) st16_stream(m.out() + 16 * g, y);
+            else if (cbytes) store_bytes(m.out() + 16 * g, y, cbytes);
+            if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
+        }
+        if (fast || valid) Y = xor4(ym, X);
     }
+    return Y;
 }
+
+// Exponent (1..32) of the power of H that aligns lane `lane`'s running value with the end of its run of rows:
+// 32 - lane for a run that ends on a full row; in the ragged last row of the message (rem = 1..32 blocks) only
+// lanes < rem folded a block there, and the lane order is rotated by rem.
+__device__ __forceinline__ uint32_t lane_exponent(uint32_t rem, uint32_t lane) { return ((rem - lane - 1) & 31) + 1; }
+
+// View of a RowMsg that lives in the kernel parameter block (constant bank): every field is a free operand.
+struct ParamMsgView {
+    const RowMsg &r;
+    __device__ __forceinline__ const uint8_t *in() const { return r.in; }
+    __device__ __forceinline__ uint8_t *out() const { return r.out; }
+    __device__ __forceinline__ const uint8_t *aad() const { return r.aad; }
+    __device__ __forceinline__ uint64_t len() const { return r.len; }
+    __device__ __forceinline__ uint64_t aad_len() const { return r.aad_len; }
+    __device__ __forceinline__ uint64_t base() const { return r.base; }
+    __device__ __forceinline__ uint64_t vblocks() const { return r.vblocks; }
+    __device__ __forceinline__ uint64_t final_len() const { return r.final_len; }
+    __device__ __forceinline__ uint64_t final_aad_len() const { return r.final_aad_len; }
+    __device__ __forceinline__ uint32_t pad() const { return r.pad; }
+    __device__ __forceinline__ uint32_t n_aad_blocks() const { return r.n_aad_blocks; }
+    __device__ __forceinline__ uint32_t fast_lo() const { return r.fast_lo; }
+    __device__ __forceinline__ uint32_t fast_hi() const { return r.fast_hi; }
+    __device__ __forceinline__ uint32_t aligned() const { return r.aligned; }
+    __device__ __forceinline__ uint32_t ctr_delta() const { return r.ctr_delta; }
+    __device__ __forceinline__ uint32_t len_block() const { return r.len_block; }
+};
+
+// View of a RowMsg in global memory: the fields the fast path touches are copied to registers once per chunk,
+// the others are loaded where the slow path needs them.
+struct GlobalMsgView {
+    const RowMsg *g;
+    const uint8_t *in_;
+    uint8_t *out_;
+    uint64_t base_;
+    uint32_t fast_lo_, fast_hi_, ctr_delta_;
+    __device__ __forceinline__ explicit GlobalMsgView(const RowMsg *p)
+        : g(p), in_(p->in), out_(p->out), base_(p->base), fast_lo_(p->fast_lo), fast_hi_(p->fast_hi), ctr_delta_(p->ctr_delta) {}
+    __device__ __forceinline__ const uint8_t *in() const { return in_; }
+    __device__ __forceinline__ uint8_t *out() const { return out_; }
+    __device__ __forceinline__ const uint8_t *aad() const { return g->aad; }
+    __device__ __forceinline__ uint64_t len() const { return g->len; }
+    __device__ __forceinline__ uint64_t aad_len() const { return g->aad_len; }
+    __device__ __forceinline__ uint64_t base() const { return base_; }
+    __device__ __forceinline__ uint64_t vblocks() const { return g->vblocks; }
+    __device__ __forceinline__ uint64_t final_len() const { return g->final_len; }
+    __device__ __forceinline__ uint64_t final_aad_len() const { return g->final_aad_len; }
+    __device__ __forceinline__ uint32_t pad() const { return g->pad; }
+    __device__ __forceinline__ uint32_t n_aad_blocks() const { return g->n_aad_blocks; }
+    __device__ __forceinline__ uint32_t fast_lo() const { return fast_lo_; }
+    __device__ __forceinline__ uint32_t fast_hi() const { return fast_hi_; }
+    __device__ __forceinline__ uint32_t aligned() const { return g->aligned; }
+    __device__ __forceinline__ uint32_t ctr_delta() const { return ctr_delta_; }
+    __device__ __forceinline__ uint32_t len_block() const { return g->len_block; }
+};
+
+// View of a RowMsg held in registers (the warp-per-message kernel derives it from its descriptor).
+struct RegMsgView {
+    RowMsg r;
+    __device__ __forceinline__ const uint8_t *in() const { return r.in; }
+    __device__ __forceinline__ uint8_t *out() const { return r.out; }
+    __device__ __forceinline__ const uint8_t *aad() const { return r.aad; }
+    __device__ __forceinline__ uint64_t len() const { return r.len; }
+    __device__ __forceinline__ uint64_t aad_len() const { return r.aad_len; }
+    __device__ __forceinline__ uint64_t base() const { return r.base; }
+    __device__ __forceinline__ uint64_t vblocks() const { return r.vblocks; }
+    __device__ __forceinline__ uint64_t final_len() const { return r.final_len; }
+    __device__ __forceinline__ uint64_t final_aad_len() const { return r.final_aad_len; }
+    __device__ __forceinline__ uint32_t pad() const { return r.pad; }
+    __device__ __forceinline__ uint32_t n_aad_blocks() const { return r.n_aad_blocks; }
+    __device__ __forceinline__ uint32_t fast_lo() const { return r.fast_lo; }
+    __device__ __forceinline__ uint32_t fast_hi() const { return r.fast_hi; }
+    __device__ __forceinline__ uint32_t aligned() const { return r.aligned; }
+    __device__ __forceinline__ uint32_t ctr_delta() const { return r.ctr_delta; }
+    __device__ __forceinline__ uint32_t len_block() const { return r.len_block; }
+};
+

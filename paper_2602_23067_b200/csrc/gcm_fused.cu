@@ -8,12 +8,13 @@
 // What differs from the paper's kernels (prior art for Ampere/Ada/Hopper):
 //   * one fused pass instead of an AES-CTR kernel followed by a GHASH kernel (the ciphertext never
 //     crosses HBM twice);
-//   * the "tree" is flattened.  The virtual block sequence [pad | AAD | payload] is cut into rows of
-//     32 blocks; a warp owns a contiguous run of rows and lane l of the warp the l-th block of each.
+//   * the "tree" is flattened.  The virtual block sequence [pad | AAD | payload | length block] is cut into
+//     rows of 32 blocks; a warp owns a contiguous run of rows and lane l of the warp the l-th block of each.
 //     Every lane therefore runs the SAME recurrence  Y <- Y.K xor X  with the one fixed multiplier
-//     K = H^32 (independent of the launch geometry and of the message), and is corrected once by
-//     H^(1..32), the warp by H^(blocks behind the warp's run), and the partials are XORed by the
-//     last CTA to finish.  The sum is the paper's sum of X_i . H^(N-i+1); only the association
+//     K = H^32 (independent of the launch geometry and of the message: the row loop of gcm_device.cuh), and is
+//     corrected once by H^(1..32); the warp sums are weighted by H^(blocks behind the warp's run) in ONE
+//     lane-parallel product by warp 0 (weights made by warp 0 while the tables arrive), and the CTA partials are
+//     XORed by the last CTA to finish.  The sum is the paper's sum of X_i . H^(N-i+1); only the association
 //     differs, and the field is exact, so the bits are identical;
 //   * the multiply by the fixed K is an 8-bit Shoup table in shared memory (conflict-free by lane
 //     rotation), AES rounds are T-tables replicated per lane (conflict-free, constant-time).  On
@@ -21,7 +22,12 @@
 //   * counters of a lane's consecutive blocks differ by 32, so for 8 rows at a time only the low
 //     counter byte changes: of rounds 1 and 2 only 1 + 4 table reads depend on it, the other 3 + 12
 //     are cached per lane and refreshed every 8th row (in addition to the 12 round-1 reads of the
-//     constant IV columns, done once per thread).
+//     constant IV columns, done once per thread);
+//   * Blackwell plumbing for the fixed cost per launch (the paper's FITS files are 17-577 MB, Table A.7,
+//     where it matters): the 64 KB multiplier table arrives by one bulk copy (TMA 1-D, cp.async.bulk) completing on
+//     an mbarrier while the threads expand the round table and warp 0 forms the position weights; the kernel is
+//     launched with programmatic stream serialization, so its prologue overlaps the previous kernel's tail and
+//     only griddepcontrol.wait orders it behind earlier work of the stream.
 //
 // Counter block of payload block g is IV || BE32(g + 2): a function of g only.
 #include "gcm_common.cuh"
@@ -30,26 +36,51 @@
 
 #include "gcm_device.cuh"
 
-// H^d for d < 2^36 from the radix-512 digit table: four factors, two multiply levels, every lane
-// of the warp takes part (lane & 3 picks the digit) and ends up with the product.
-__device__ __forceinline__ uint4 warp_h_power(const uint4 *hx, uint64_t d, uint32_t lane, uint64_t d_max)
+#include <atomic>
+#include <stdlib.h>
+
+#define STAMP(k)                                                                                   \
+    do {                                                                                           \
+        if (p.stamps != nullptr && threadIdx.x == 0) p.stamps[8 * blockIdx.x + (k)] = global_timer_ns(); \
+    } while (0)
+
+__device__ __forceinline__ uint4 warp_xor4(uint4 v)
 {
-    const uint32_t k = lane & 3;
-    const uint32_t digit = (uint32_t)(d >> (HX_RADIX_BITS * k)) & ((1u << HX_RADIX_BITS) - 1);
-    uint4 f = __ldg(hx + (k << HX_RADIX_BITS) + digit);
-    // d_max (launch-uniform bound on d) says how many digits can be non-zero: short messages skip levels
-    const int levels = d_max < (1ull << HX_RADIX_BITS) ? 0 : (d_max < (1ull << (2 * HX_RADIX_BITS)) ? 1 : 2);
-    for (int o = 1; o <= levels; o++) {
-        const int m = 1 << (o - 1);
-        uint4 g;
-        g.x = __shfl_xor_sync(0xFFFFFFFFu, f.x, m); g.y = __shfl_xor_sync(0xFFFFFFFFu, f.y, m);
-        g.z = __shfl_xor_sync(0xFFFFFFFFu, f.z, m); g.w = __shfl_xor_sync(0xFFFFFFFFu, f.w, m);
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        v.x ^= __shfl_xor_sync(0xFFFFFFFFu, v.x, o); v.y ^= __shfl_xor_sync(0xFFFFFFFFu, v.y, o);
+        v.z ^= __shfl_xor_sync(0xFFFFFFFFu, v.z, o); v.w ^= __shfl_xor_sync(0xFFFFFFFFu, v.w, o);
+    }
+    return v;
+}
+
+// a8, first half, by warp 0 while the multiplier table is still on its way: D_w = H^(blocks behind the run of
+// warp w of this CTA) for every warp of the CTA at once.  H^d for d < 2^36 is a product of four entries of the
+// radix-512 digit table (PAPER.md L197 precomputes H^(2^k): 36 factors; radix 512 needs 4).  Lane j works for
+// warp j >> 1 on digit pair j & 1, so the two product levels serve all (up to 16) warps in two generic products;
+// messages below 2^18 / 2^9 blocks need one / none.  The tail run and runs without rows get H^0 = 1.
+template <int NW>
+__device__ __forceinline__ void cta_position_weights(const GcmParams &p, uint32_t lane, uint4 *wpow)
+{
+    const uint64_t E = p.m.vblocks;
+    const uint32_t S = p.m.rows, w = lane >> 1, half = lane & 1;
+    const uint64_t wg = (uint64_t)blockIdx.x * NW + w;
+    const uint32_t r1 = (uint32_t)(((wg + 1) * S) / p.warps);
+    const uint64_t d = (w < NW && r1 < S) ? E - 32ull * r1 : 0;
+    const int levels = E < (1ull << HX_RADIX_BITS) ? 0 : (E < (1ull << (2 * HX_RADIX_BITS)) ? 1 : 2);
+    const uint32_t k0 = 2 * half, k1 = 2 * half + 1, mask = (1u << HX_RADIX_BITS) - 1;
+    uint4 f = __ldg(p.tab.hx + (k0 << HX_RADIX_BITS) + ((uint32_t)(d >> (HX_RADIX_BITS * k0)) & mask));
+    if (levels >= 1) {
+        const uint4 g = __ldg(p.tab.hx + (k1 << HX_RADIX_BITS) + ((uint32_t)(d >> (HX_RADIX_BITS * k1)) & mask));
         f = gf_mul_mem(f, g);
     }
-    // lanes with k = 0 hold the product of the digits that can be non-zero; hand it to every lane
-    f.x = __shfl_sync(0xFFFFFFFFu, f.x, lane & ~3u); f.y = __shfl_sync(0xFFFFFFFFu, f.y, lane & ~3u);
-    f.z = __shfl_sync(0xFFFFFFFFu, f.z, lane & ~3u); f.w = __shfl_sync(0xFFFFFFFFu, f.w, lane & ~3u);
-    return f;
+    if (levels == 2) {
+        uint4 g;
+        g.x = __shfl_xor_sync(0xFFFFFFFFu, f.x, 1); g.y = __shfl_xor_sync(0xFFFFFFFFu, f.y, 1);
+        g.z = __shfl_xor_sync(0xFFFFFFFFu, f.z, 1); g.w = __shfl_xor_sync(0xFFFFFFFFu, f.w, 1);
+        f = gf_mul_mem(f, g);
+    }
+    if (half == 0 && w < NW) wpow[w] = f;
 }
 
 template <int NR, int MODE, int TPB>
@@ -57,158 +88,97 @@ __global__ void __launch_bounds__(TPB, 1)
 gcm_fused_kernel(const __grid_constant__ GcmParams p)
 {
     extern __shared__ __align__(1024) uint8_t sm[];
-    __shared__ bool s_last;
     __shared__ uint4 s_ekj0;
+    constexpr uint32_t NW = TPB / 32;
     const uint32_t t = threadIdx.x, lane = t & 31, lane4 = lane * 4;
-    // broadcast from lane 0: tells the compiler the warp index (and the row loop below) is warp-uniform,
+    // broadcast from lane 0: tells the compiler the warp index (and the row loop) is warp-uniform,
     // so the shared-memory base stays in a uniform register and folds into every LDS address
     const uint32_t warp = __shfl_sync(0xFFFFFFFFu, t >> 5, 0);
     uint4 *red = reinterpret_cast<uint4 *>(sm + RED_OFF);
+    uint4 *wpow = reinterpret_cast<uint4 *>(sm + WPOW_OFF);
 
-    // this warp's run of rows (a8: geometry-agnostic, the result does not depend on it)
-    const uint32_t S = p.rows, Q = p.rows_per_warp;
-    const uint64_t wg = (uint64_t)blockIdx.x * (TPB / 32) + warp;
-    const uint64_t r0_64 = wg * Q;
-    const uint32_t r0 = r0_64 < S ? (uint32_t)r0_64 : S;
-    const uint32_t r1 = (uint64_t)r0 + Q < S ? r0 + Q : S;
+    pdl_launch_dependents();            // the next launch of the stream may begin its own prologue
+    STAMP(0);
+    tables_begin<TPB, MODE != MODE_GHASH, true>(sm, p.tab, p.te0);
+
+    // this warp's run of rows (geometry-agnostic: the result does not depend on it), balanced to +-1 row
+    const uint32_t S = p.m.rows;
+    const uint64_t wg = (uint64_t)blockIdx.x * NW + warp;
+    // (the broadcasts keep the loop bounds in uniform registers: the 64-bit divisions hide from the compiler that
+    // they are warp-uniform, and a row loop it takes for divergent cannot fold the shared-memory base into its LDS)
+    const uint32_t r0 = __shfl_sync(0xFFFFFFFFu, (uint32_t)((wg * S) / p.warps), 0);
+    const uint32_t r1 = __shfl_sync(0xFFFFFFFFu, (uint32_t)(((wg + 1) * S) / p.warps), 0);
     const bool has_rows = r0 < r1;
 
-    {
-        KtabRegs<TPB> kr;
-        ktab_load<TPB>(kr, p.tab.ktab);
-        if (MODE != MODE_GHASH) fill_aes_tables<TPB>(sm, p.tab.te0);
-        ktab_store<TPB>(kr, sm);
-    }
-    const bool tail_warp = has_rows && r1 == S;          // owns the last (possibly ragged) row
-    __syncthreads();
+    tables_wait(sm);
+    STAMP(1);
+    // a8, first half: only warp 0 reads the position weights (after the rows), so only warp 0 forms them, and the
+    // other warps do not wait for it: under programmatic dependent launch this falls into the wait for the previous
+    // kernel of the stream; in an isolated launch warp 0 starts its rows two generic products late
+    if (warp == 0) cta_position_weights<NW>(p, lane, wpow);
+    STAMP(7);
 
-    uint32_t sel[8];
-#pragma unroll
-    for (int r = 0; r < 8; r++) sel[r] = ((lane + r) & 7) << 4;
+    const MulK8 mul(sm, lane);
     CtrConst cc = {0, 0, 0, 0};
-    CtrCache cu = {0, 0, 0, 0};
     if (MODE != MODE_GHASH) {
         cc = ctr_const(p.rk, p.iv[0], p.iv[1], p.iv[2], sm, lane4);
         // a3: E_K(J0), J0 = IV || 0^31 || 1, by the last warp of every CTA while the others start their rows
         // (any CTA may turn out to be the finisher); it reaches the finishing thread through shared memory
-        if (warp == TPB / 32 - 1) {
+        if (warp == NW - 1) {
             const CtrCache c1 = ctr_cache(p.rk, sm, lane4, cc, 1u);
             const uint4 ek = aes_ctr_block<NR>(p.rk, sm, lane4, cc, c1, 1u);
             if (lane == 0) s_ekj0 = ek;
         }
     }
+    // Nothing above depends on earlier work of the stream (tables are per key and complete before gcm_init
+    // returns); payload, AAD, partials, ticket and verdict do.
+    pdl_wait();
+    STAMP(2);
+    if (MODE == MODE_DECRYPT && p.status_init && blockIdx.x == 0 && t == 0) *p.status = GCM_STATUS_PENDING;
 
-    uint4 Y = make_uint4(0, 0, 0, 0);
-    uint4 pre = make_uint4(0, 0, 0, 0);
-    bool have_pre = false;
+    const ParamMsgView m{p.m};
+    const uint4 Y = gcm_rows<NR, MODE>(m, p.rk, sm, lane, cc, r0, r1, mul);      // a4-a7
+    STAMP(3);
 
-    // a8, first half: the weight each lane's partial is multiplied by at the end of the run,
-    //     V_l = H^(blocks from the lane's last block to the end of the run) . H^(blocks behind the run).
-    // In the ragged last row only lanes < rem folded a block; rotating the lane order by rem keeps the first
-    // exponent in 1..32.  The generic products behind V (up to three per warp) are NOT done before the rows or
-    // after them, where all warps of the SM would do them at once with the table pipe idle, but in the middle
-    // of the run, at a row that differs from warp to warp: the other warps keep the shared-memory pipe busy.
-    uint4 V = make_uint4(0, 0, 0, 0);
-    const uint32_t rmid = r0 + (uint32_t)(((uint64_t)(r1 - r0) * (warp + 1)) / (TPB / 32 + 1));
-
-    for (uint32_t row = r0; row < r1; row++) {
-        if (row == rmid) {                               // once per run, at a warp-specific row (see above)
-            const uint32_t rem = tail_warp ? (uint32_t)(p.vblocks - 32ull * (S - 1)) : 32u;   // 1..32
-            V = __ldg(p.tab.hpow + (((rem - lane - 1) & 31) + 1));
-            if (!tail_warp) V = gf_mul_mem(V, warp_h_power(p.tab.hx, p.vblocks - 32ull * r1, lane, p.vblocks));
-        }
-        const uint64_t v = 32ull * row + lane;          // virtual block index
-        const bool fast = row >= p.fast_lo && row < p.fast_hi;
-        uint4 x = make_uint4(0, 0, 0, 0);
-        uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD / beyond the end)
-        uint64_t g = 0;                                 // payload block index
-        bool valid = true;
-        if (fast) {
-            g = v - p.base;
-            x = have_pre ? pre : ld16_stream(p.in + 16 * g);
-            cbytes = 16;
-            have_pre = row + 1 < r1 && row + 1 < p.fast_hi;
-            if (have_pre) pre = ld16_stream(p.in + 16 * g + 512);
-        } else {
-            have_pre = false;
-            valid = v < p.vblocks;
-            if (valid && v >= p.pad) {
-                const uint64_t u = v - p.pad;
-                if (u < p.n_aad_blocks) {
-                    const uint64_t rem = p.aad_len - 16 * u;
-                    x = load_bytes(p.aad + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
-                } else {
-                    g = u - p.n_aad_blocks;
-                    const uint64_t rem = p.len - 16 * g;
-                    cbytes = rem < 16 ? (uint32_t)rem : 16u;
-                    x = (cbytes == 16 && p.aligned) ? ld16_stream(p.in + 16 * g) : load_bytes(p.in + 16 * g, cbytes);
-                }
-            }
-        }
-        // a7: multiply the running value by K; independent of this row's AES, so they interleave
-        const uint4 ym = ghash_mul_k(sm, sel, Y);
-        uint4 X = x;
-        if (MODE != MODE_GHASH) {
-            // a4: counter from the virtual index alone; the upper 24 bits are warp-uniform and change
-            // every 8th row, when rounds 1-2 are re-cached
-            const uint32_t ctr = (uint32_t)v + p.ctr_delta;
-            if (row == r0 || (ctr & 0xE0u) == 0) cu = ctr_cache(p.rk, sm, lane4, cc, ctr);
-            const uint4 ks = aes_ctr_block<NR>(p.rk, sm, lane4, cc, cu, ctr);     // a5
-            const uint4 y = xor4(x, ks);                                   // a6
-            if (cbytes == 16 && (fast || p.aligned)) st16_stream(p.out + 16 * g, y);
-            else if (cbytes) store_bytes(p.out + 16 * g, y, cbytes);
-            if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
-        }
-        if (fast || valid) Y = xor4(ym, X);
-    }
-    // a8, second half: one product per lane, XOR over the warp, XOR over the CTA
+    // a8, second half: one product per lane aligns it with the end of the warp's run, XOR over the warp;
+    // warp 0 then weights the warp sums with their positions (one lane-parallel product) and XORs them
     uint4 part = make_uint4(0, 0, 0, 0);
-    if (has_rows) part = gf_mul_mem(Y, V);
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) {
-        part.x ^= __shfl_xor_sync(0xFFFFFFFFu, part.x, o); part.y ^= __shfl_xor_sync(0xFFFFFFFFu, part.y, o);
-        part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
+    if (has_rows) {
+        const uint32_t rem = r1 == S ? (uint32_t)(p.m.vblocks - 32ull * (S - 1)) : 32u;       // 1..32
+        part = gf_mul_mem(Y, __ldg(p.tab.hpow + lane_exponent(rem, lane)));
     }
+    part = warp_xor4(part);
     if (lane == 0) red[warp] = part;
     __syncthreads();
-    if (warp == 0) {
-        part = lane < TPB / 32 ? red[lane] : make_uint4(0, 0, 0, 0);
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) {
-            part.x ^= __shfl_xor_sync(0xFFFFFFFFu, part.x, o); part.y ^= __shfl_xor_sync(0xFFFFFFFFu, part.y, o);
-            part.z ^= __shfl_xor_sync(0xFFFFFFFFu, part.z, o); part.w ^= __shfl_xor_sync(0xFFFFFFFFu, part.w, o);
-        }
-    }
-    // a9: last-CTA-done combination of the partials
-    if (t == 0) {
-        p.partials[blockIdx.x] = part;
+    STAMP(4);
+    if (warp != 0) return;
+    uint4 acc = make_uint4(0, 0, 0, 0), wgt = make_uint4(0, 0, 0, 0);
+    if (lane < NW) { acc = red[lane]; wgt = wpow[lane]; }
+    acc = warp_xor4(gf_mul_mem(acc, wgt));
+    // a9: last-CTA-done combination of the CTA partials.  The ticket counter is never reset: the host hands
+    // every launch the ticket value that ends it, so an aborted launch cannot leave a stale count behind.
+    unsigned ticket = 0;
+    if (lane == 0) {
+        p.partials[blockIdx.x] = acc;
         __threadfence();
-        const unsigned ticket = atomicAdd(p.counter, 1u);
-        s_last = (ticket == gridDim.x - 1);
+        ticket = atomicAdd(p.counter, 1u);
     }
-    __syncthreads();
-    if (!s_last) return;
+    ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
+    STAMP(5);
+    if (ticket != p.ticket_last) return;
     __threadfence();
-    uint4 acc = make_uint4(0, 0, 0, 0);
-    for (uint32_t j = t; j < gridDim.x; j += TPB) acc = xor4(acc, __ldcg(p.partials + j));
-    acc = cta_xor_reduce(acc, red);
-    if (t == 0) {
-        if (p.chain_in != nullptr) acc = xor4(acc, gf_mul_mem(*p.chain_in, *p.chain_pow));
+    uint4 tot = make_uint4(0, 0, 0, 0);
+    for (uint32_t j = lane; j < gridDim.x; j += 32) tot = xor4(tot, __ldcg(p.partials + j));
+    tot = warp_xor4(tot);
+    if (lane == 0) {
+        if (p.chain_in != nullptr) tot = xor4(tot, gf_mul_mem(*p.chain_in, *p.chain_pow));
         if (p.chain_out != nullptr) {       // a middle chunk of a longer message: hand the state on
-            *p.chain_out = acc;
-            *p.counter = 0;
-            return;
-        }
-        // a10: length block BE64(8a) || BE64(8 len), one more multiply by H
-        const uint64_t abits = p.final_aad_len * 8, cbits = p.final_len * 8;
-        const uint4 L = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
-                                   bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
-        const uint4 Sg = gf_mul_mem(xor4(acc, L), __ldg(p.tab.h));
-        if (MODE == MODE_GHASH) {
-            *p.tag_out = Sg;
+            *p.chain_out = tot;
+        } else if (MODE == MODE_GHASH) {     // a10 is part of the rows: tot is GHASH_H(A, C)
+            *p.tag_out = tot;
         } else {
             // a11: tag = E_K(J0) xor S; constant-time compare
-            const uint4 tag = xor4(Sg, s_ekj0);
+            const uint4 tag = xor4(tot, s_ekj0);
             if (MODE == MODE_ENCRYPT) {
                 *p.tag_out = tag;
             } else {
@@ -218,26 +188,58 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
                 *p.status = diff != 0 ? 1 : 0;
             }
         }
-        *p.counter = 0;   // ready for the next launch on this context
     }
+    STAMP(6);
 }
 
 // ---- host side ------------------------------------------------------------------------------------
-template <int NR, int MODE, int TPB>
-static cudaError_t launch_one(int blocks, const GcmParams &p, cudaStream_t s)
+// Programmatic stream serialization (on unless GCM_NO_PDL is set in the environment, for A/B measurements).
+static bool pdl_enabled()
 {
-    static bool configured[64] = {false};   // per instantiation and device; the attribute is sticky
-    auto kern = gcm_fused_kernel<NR, MODE, TPB>;
+    static const bool on = getenv("GCM_NO_PDL") == nullptr;
+    return on;
+}
+
+cudaError_t launch_with_pdl(const void *kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, void **args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelExC(&cfg, kern, args);
+}
+
+// The opt-in shared-memory size is a sticky per-function, per-device attribute: set once per (function, device).
+cudaError_t ensure_smem_attr(const void *kern, std::atomic<bool> *configured, size_t bytes)
+{
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64 || !configured[dev]) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FUSED_SMEM_BYTES);
+    const bool tracked = dev >= 0 && dev < GCM_MAX_DEVICES;
+    if (!tracked || !configured[dev].load(std::memory_order_acquire)) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) configured[dev] = true;
+        if (tracked) configured[dev].store(true, std::memory_order_release);      // setting it twice is harmless
     }
-    kern<<<blocks, TPB, FUSED_SMEM_BYTES, s>>>(p);
-    return cudaGetLastError();
+    return cudaSuccess;
+}
+
+template <int NR, int MODE, int TPB>
+static cudaError_t launch_one(int blocks, const GcmParams &p, cudaStream_t s)
+{
+    static std::atomic<bool> configured[GCM_MAX_DEVICES];   // per instantiation and device
+    const void *kern = (const void *)gcm_fused_kernel<NR, MODE, TPB>;
+    cudaError_t e = ensure_smem_attr(kern, configured, FUSED_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    void *args[] = {(void *)&p};
+    return launch_with_pdl(kern, dim3(blocks), dim3(TPB), FUSED_SMEM_BYTES, s, args);
 }
 
 template <int TPB>

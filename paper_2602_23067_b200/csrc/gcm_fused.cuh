@@ -10,3 +10,10 @@ cudaError_t launch_fused(int nr, int mode, int threads, int blocks, const GcmPar
 // (AAD blocks + payload blocks + the length block); MODE_ENCRYPT / MODE_DECRYPT only, no chunk chaining.
 #define SMALL_MAX_BLOCKS 511
 cudaError_t launch_small(int nr, int mode, const GcmParams &p, cudaStream_t s);
+
+// gcm_fused.cu: shared launch helpers.  launch_with_pdl launches with programmatic stream serialization (the
+// kernel must call griddepcontrol.wait before it touches stream-ordered data); ensure_smem_attr raises the
+// dynamic shared-memory limit of `kern` once per device (configured: GCM_MAX_DEVICES flags owned by the caller).
+#include <atomic>
+cudaError_t launch_with_pdl(const void *kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, void **args);
+cudaError_t ensure_smem_attr(const void *kern, std::atomic<bool> *configured, size_t bytes);

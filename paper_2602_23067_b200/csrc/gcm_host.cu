@@ -34,13 +34,12 @@
 struct HostPipe {
     cudaStream_t stream[PIPE_SLOTS];
     cudaEvent_t kernel_done[PIPE_SLOTS];
-    cudaEvent_t slot_free[PIPE_SLOTS];
     cudaEvent_t start;
     uint8_t *d_stage[PIPE_SLOTS];
     uint8_t *d_aad;
     size_t aad_cap;
     uint4 *d_state;     // [2]: running GHASH state, ping-pong
-    uint4 *d_pows;      // [2]: H^(blocks of a full chunk), H^(blocks of the last chunk)
+    uint4 *d_pows;      // [2]: H^(blocks of a full chunk), H^(blocks of the last chunk + the length block)
 };
 
 #define CU(call)                                                                                   \
@@ -62,22 +61,48 @@ __global__ void gcm_pow_kernel(const uint4 *h, uint64_t e0, uint64_t e1, uint4 *
     out[threadIdx.x] = gf_to_mem(r);
 }
 
+static void pipe_destroy(HostPipe *hp)
+{
+    if (!hp) return;
+    for (int i = 0; i < PIPE_SLOTS; i++) {
+        if (hp->stream[i]) cudaStreamSynchronize(hp->stream[i]);
+        if (hp->d_stage[i]) {
+            launch_wipe(hp->d_stage[i], PIPE_CHUNK_BYTES, nullptr, 0);
+            cudaDeviceSynchronize();
+            cudaFree(hp->d_stage[i]);
+        }
+        if (hp->kernel_done[i]) cudaEventDestroy(hp->kernel_done[i]);
+        if (hp->stream[i]) cudaStreamDestroy(hp->stream[i]);
+    }
+    if (hp->start) cudaEventDestroy(hp->start);
+    if (hp->d_aad) cudaFree(hp->d_aad);
+    if (hp->d_state) cudaFree(hp->d_state);
+    cudaGetLastError();
+    delete hp;
+}
+
+// The pipeline is built in a local and attached to the context only when complete: a failed allocation (192 MiB
+// of staging) leaves the context as it was, and the next call tries again.
 static int pipe_get(gcm_ctx *c, size_t aad_len)
 {
     if (!c->pipe) {
         HostPipe *hp = new (std::nothrow) HostPipe;
         if (!hp) return GCM_ERR_NOMEM;
         memset(hp, 0, sizeof(*hp));
-        c->pipe = hp;
-        for (int i = 0; i < PIPE_SLOTS; i++) {
-            CU(cudaStreamCreateWithFlags(&hp->stream[i], cudaStreamNonBlocking));
-            CU(cudaEventCreateWithFlags(&hp->kernel_done[i], cudaEventDisableTiming));
-            CU(cudaEventCreateWithFlags(&hp->slot_free[i], cudaEventDisableTiming));
-            CU(cudaMalloc((void **)&hp->d_stage[i], PIPE_CHUNK_BYTES));
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < PIPE_SLOTS && e == cudaSuccess; i++) {
+            if ((e = cudaStreamCreateWithFlags(&hp->stream[i], cudaStreamNonBlocking)) != cudaSuccess) break;
+            if ((e = cudaEventCreateWithFlags(&hp->kernel_done[i], cudaEventDisableTiming)) != cudaSuccess) break;
+            e = cudaMalloc((void **)&hp->d_stage[i], PIPE_CHUNK_BYTES);
         }
-        CU(cudaEventCreateWithFlags(&hp->start, cudaEventDisableTiming));
-        CU(cudaMalloc((void **)&hp->d_state, 4 * sizeof(uint4)));
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->start, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&hp->d_state, 4 * sizeof(uint4));
+        if (e != cudaSuccess) {
+            pipe_destroy(hp);
+            return gcm_cuda_fail(e);
+        }
         hp->d_pows = hp->d_state + 2;
+        c->pipe = hp;
     }
     HostPipe *hp = c->pipe;
     if (aad_len > hp->aad_cap) {
@@ -93,36 +118,20 @@ static int pipe_get(gcm_ctx *c, size_t aad_len)
 
 void gcm_host_pipe_free(gcm_ctx *c)
 {
-    HostPipe *hp = c->pipe;
-    if (!hp) return;
-    for (int i = 0; i < PIPE_SLOTS; i++) {
-        if (hp->stream[i]) cudaStreamSynchronize(hp->stream[i]);
-        if (hp->d_stage[i]) {
-            launch_wipe(hp->d_stage[i], PIPE_CHUNK_BYTES, nullptr, 0);
-            cudaDeviceSynchronize();
-            cudaFree(hp->d_stage[i]);
-        }
-        if (hp->kernel_done[i]) cudaEventDestroy(hp->kernel_done[i]);
-        if (hp->slot_free[i]) cudaEventDestroy(hp->slot_free[i]);
-        if (hp->stream[i]) cudaStreamDestroy(hp->stream[i]);
-    }
-    if (hp->start) cudaEventDestroy(hp->start);
-    if (hp->d_aad) cudaFree(hp->d_aad);
-    if (hp->d_state) cudaFree(hp->d_state);
-    delete hp;
+    pipe_destroy(c->pipe);
     c->pipe = nullptr;
 }
 
 // d_sum32 (device, may be NULL): every chunk's ciphertext is also added to the FITS DATASUM accumulator
 // while it is still in the staging buffer (the container layer of gfc_frame.cu).
+// mode MODE_GHASH: the chunks are only hashed (no AES, nothing copied back): tag_io receives GHASH_H(A, C).
 int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uint64_t aad_len,
                  const void *h_in, uint64_t len, void *h_out, uint8_t *tag_io, void *user_stream,
                  unsigned long long *d_sum32)
 {
-    if (!c || !iv || !tag_io) return GCM_ERR_ARG;
+    if (!c || (!iv && mode != MODE_GHASH) || !tag_io) return GCM_ERR_ARG;
     if (len > ((1ull << 36) - 32) || aad_len >= (1ull << 32)) return GCM_ERR_LEN;
-    if ((aad_len && !h_aad) || (len && (!h_in || !h_out))) return GCM_ERR_ARG;
-    CU(cudaSetDevice(c->device));
+    if ((aad_len && !h_aad) || (len && (!h_in || (!h_out && mode != MODE_GHASH)))) return GCM_ERR_ARG;
     int rc = pipe_get(c, aad_len);
     if (rc != GCM_OK) return rc;
     HostPipe *hp = c->pipe;
@@ -140,10 +149,14 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
     for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamWaitEvent(hp->stream[i], hp->start, 0));
     if (aad_len) CU(cudaMemcpyAsync(hp->d_aad, h_aad, aad_len, cudaMemcpyHostToDevice, hp->stream[0]));
     if (n_chunks > 1) {
-        gcm_pow_kernel<<<1, 2, 0, hp->stream[PIPE_SLOTS - 1]>>>(c->d_h, chunk / 16, (last_len + 15) / 16, hp->d_pows);
+        // GHASH blocks per chunk: a middle chunk's payload blocks; the last chunk's plus the length block
+        gcm_pow_kernel<<<1, 2, 0, hp->stream[PIPE_SLOTS - 1]>>>(c->d_h, chunk / 16, (last_len + 15) / 16 + 1, hp->d_pows);
         CU(cudaGetLastError());
         CU(cudaEventRecord(hp->kernel_done[PIPE_SLOTS - 1], hp->stream[PIPE_SLOTS - 1]));
     }
+    // the verdict reads "refused" until the finisher of the last chunk has written it (fail closed)
+    volatile int *verdict = (volatile int *)(c->h_pinned + 16);
+    *verdict = GCM_STATUS_PENDING;
 
     for (uint64_t k = 0; k < n_chunks; k++) {
         const int slot = (int)(k % PIPE_SLOTS);
@@ -159,50 +172,102 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         GcmParams p;
         int blocks = 0;
         rc = gcm_build_params(c, mode, iv, first ? hp->d_aad : nullptr, first ? aad_len : 0,
-                              hp->d_stage[slot], clen, hp->d_stage[slot], (uint32_t)(off / 16), &p, &blocks);
+                              hp->d_stage[slot], clen, mode == MODE_GHASH ? nullptr : hp->d_stage[slot],
+                              (uint32_t)(off / 16), last, len, aad_len, &p, &blocks);
         if (rc != GCM_OK) return rc;
-        p.final_len = len;
-        p.final_aad_len = aad_len;
         if (!first) {
             p.chain_in = hp->d_state + ((k - 1) & 1);
             p.chain_pow = hp->d_pows + (last ? 1 : 0);
         }
         if (!last) p.chain_out = hp->d_state + (k & 1);
         if (mode == MODE_DECRYPT) memcpy(p.tag_expect, tag_io, 16);
-        cudaError_t e = launch_fused(c->nr, mode, c->threads, blocks, p, s);
+        // tag / verdict of the last chunk go straight into mapped pinned host memory
+        p.tag_out = (uint4 *)c->h_pinned;
+        p.status = (int *)(c->h_pinned + 16);
+        cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s);
         memset(&p, 0, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
         CU(cudaEventRecord(hp->kernel_done[slot], s));
         if (d_sum32 && mode == MODE_ENCRYPT) CU(launch_fits_sum32(hp->d_stage[slot], clen, d_sum32, c->sm_count, s));
-        if (clen) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
-        if (last) {
-            if (mode == MODE_ENCRYPT) CU(cudaMemcpyAsync(c->h_pinned, c->d_tag, 16, cudaMemcpyDeviceToHost, s));
-            else CU(cudaMemcpyAsync(c->h_pinned + 16, c->d_status, 4, cudaMemcpyDeviceToHost, s));
-        }
+        if (clen && mode != MODE_GHASH) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
     }
     for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamSynchronize(hp->stream[i]));
-    if (mode == MODE_ENCRYPT) {
+    if (mode != MODE_DECRYPT) {
         memcpy(tag_io, c->h_pinned, 16);
         return GCM_OK;
     }
-    int status;
-    memcpy(&status, c->h_pinned + 16, 4);
-    if (status != 0) {
+    if (*verdict != 0) {
         memset(h_out, 0, len);       // payload suppression on the host copy
         return GCM_ERR_AUTH;
     }
     return GCM_OK;
 }
 
+#define LOCK_CTX(c)                                                                                \
+    if (!(c)) return GCM_ERR_ARG;                                                                  \
+    CtxLock lock__(c);                                                                             \
+    if (!lock__.ok) return GCM_ERR_BUSY;                                                           \
+    DeviceGuard guard__((c)->device);                                                              \
+    CU(guard__.err)
+
 extern "C" int gcm_encrypt_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
                                 const void *h_pt, uint64_t len, void *h_ct, uint8_t tag[16], void *stream)
 {
+    LOCK_CTX(c);
     return gcm_host_run(c, MODE_ENCRYPT, iv, h_aad, aad_len, h_pt, len, h_ct, tag, stream, nullptr);
 }
 
 extern "C" int gcm_decrypt_verify_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
                                        const void *h_ct, uint64_t len, void *h_pt, const uint8_t tag[16], void *stream)
 {
+    if (!tag) return GCM_ERR_ARG;
+    LOCK_CTX(c);
+    uint8_t t[16];
+    memcpy(t, tag, 16);
+    return gcm_host_run(c, MODE_DECRYPT, iv, h_aad, aad_len, h_ct, len, h_pt, t, stream, nullptr);
+}
+
+// E_K(J0) xor S compared with the expected tag on the device (constant time), verdict into mapped pinned memory.
+__global__ void gcm_tag_check_kernel(const uint4 *ekj0, const uint4 *s, uint4 expect, int *status)
+{
+    const uint4 t = xor4(*ekj0, *s);
+    const uint32_t diff = (t.x ^ expect.x) | (t.y ^ expect.y) | (t.z ^ expect.z) | (t.w ^ expect.w);
+    *status = diff != 0 ? 1 : 0;
+}
+
+extern "C" int gcm_decrypt_verify_host_strict(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
+                                              const void *h_ct, uint64_t len, void *h_pt, const uint8_t tag[16], void *stream)
+{
+    if (!tag || !iv) return GCM_ERR_ARG;
+    LOCK_CTX(c);
+    // pass 1: S = GHASH_H(A, C) over the host buffer (H2D + GHASH-only kernel per chunk, no AES, no output)
+    uint8_t s_host[16];
+    int rc = gcm_host_run(c, MODE_GHASH, nullptr, h_aad, aad_len, h_ct, len, nullptr, s_host, stream, nullptr);
+    if (rc != GCM_OK) return rc;
+    // E_K(J0) = tag of the empty message with empty AAD (S = 0) through the latency kernel; compare on the device
+    HostPipe *hp = c->pipe;
+    cudaStream_t s = hp->stream[0];
+    {
+        GcmParams p;
+        int blocks = 0;
+        rc = gcm_build_params(c, MODE_ENCRYPT, iv, nullptr, 0, nullptr, 0, nullptr, 0, true, 0, 0, &p, &blocks);
+        if (rc != GCM_OK) return rc;
+        c->ticket_next -= (unsigned)blocks;                      // the latency kernel draws no tickets
+        p.tag_out = hp->d_state;                                 // E_K(J0)
+        cudaError_t e = launch_small(c->nr, MODE_ENCRYPT, p, s);
+        memset(&p, 0, sizeof(p));
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+    }
+    CU(cudaMemcpyAsync(hp->d_state + 1, s_host, 16, cudaMemcpyHostToDevice, s));
+    volatile int *verdict = (volatile int *)(c->h_pinned + 16);
+    *verdict = GCM_STATUS_PENDING;
+    uint4 expect;
+    memcpy(&expect, tag, 16);
+    gcm_tag_check_kernel<<<1, 1, 0, s>>>(hp->d_state, hp->d_state + 1, expect, (int *)(c->h_pinned + 16));
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(s));
+    if (*verdict != 0) return GCM_ERR_AUTH;                      // nothing was written to h_pt
+    // pass 2: the ordinary pipeline (which verifies once more while it decrypts)
     uint8_t t[16];
     memcpy(t, tag, 16);
     return gcm_host_run(c, MODE_DECRYPT, iv, h_aad, aad_len, h_ct, len, h_pt, t, stream, nullptr);

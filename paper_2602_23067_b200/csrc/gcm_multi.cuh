@@ -5,25 +5,14 @@
 #include <stdint.h>
 #include "gcm_common.cuh"
 
-// One message of the group, device memory.  Same virtual block sequence as the single-message kernel
-// (gcm_common.cuh): [pad zero blocks | AAD blocks | payload blocks], rows of 32.
+// One message of the group, device memory: the row loop's view of it (gcm_common.cuh: RowMsg, the same virtual
+// block sequence [pad | AAD | payload | length block] as the single-message kernel) plus IV, expected tag and the
+// slot its result goes to.
 struct MultiMsg {
+    RowMsg   m;
     uint32_t iv[3];
-    uint32_t pad;             // leading virtual zero blocks
-    const uint8_t *in;
-    uint8_t       *out;
-    const uint8_t *aad;
-    uint64_t len, aad_len;
-    uint64_t base;            // pad + AAD blocks
-    uint64_t vblocks;         // E
-    uint32_t n_aad_blocks;
-    uint32_t rows;            // S
-    uint32_t fast_lo, fast_hi;
-    uint32_t aligned;
-    uint32_t ctr_delta;
-    uint32_t tag_expect[4];   // decrypt
     uint32_t result;          // index into the result array
-    uint32_t reserved;
+    uint32_t tag_expect[4];   // decrypt
 };
 
 // Rows [r0, r1) of message msg: the unit of work of one warp.  Warp w owns chunks
@@ -34,6 +23,7 @@ struct MultiResult { uint32_t tag[4]; int status; int pad[3]; };   // == BatchRe
 
 struct MultiParams {
     uint32_t rk[60];
+    uint32_t te0[256];        // round table T0 (see GcmParams)
     GcmTables tab;
     const MultiMsg   *msgs;
     const MultiChunk *chunks;

@@ -30,8 +30,10 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
     const uint32_t t = threadIdx.x, lane = t & 31, lane4 = lane * 4, warp = t >> 5;
     uint4 *red = reinterpret_cast<uint4 *>(sm + AES_TAB_BYTES);
 
-    const uint32_t n_aad = p.n_aad_blocks;
-    const uint32_t n_c = (uint32_t)((p.len + 15) / 16);
+    pdl_launch_dependents();
+    pdl_wait();             // the payload loads below come first: nothing worth overlapping ahead of them
+    const uint32_t n_aad = p.m.n_aad_blocks;
+    const uint32_t n_c = (uint32_t)((p.m.len + 15) / 16);
     const uint32_t N = n_aad + n_c + 1;                       // <= SMALL_MAX_BLOCKS
 
     // this thread's blocks (at most two) and their weights: global loads go out before the table fill
@@ -46,21 +48,21 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
         if (i >= N) continue;
         w[k] = __ldg(p.tab.hx + (N - i));                     // H^(N - i), exponent 1 .. 511
         if (i < n_aad) {
-            const uint64_t rem = p.aad_len - 16ull * i;
-            x[k] = load_bytes(p.aad + 16ull * i, rem < 16 ? (uint32_t)rem : 16u);
+            const uint64_t rem = p.m.aad_len - 16ull * i;
+            x[k] = load_bytes(p.m.aad + 16ull * i, rem < 16 ? (uint32_t)rem : 16u);
         } else if (i < N - 1) {
             const uint32_t g = i - n_aad;
-            const uint64_t rem = p.len - 16ull * g;
+            const uint64_t rem = p.m.len - 16ull * g;
             cbytes[k] = rem < 16 ? (uint32_t)rem : 16u;
-            x[k] = (cbytes[k] == 16 && p.aligned) ? ld16_stream(p.in + 16ull * g) : load_bytes(p.in + 16ull * g, cbytes[k]);
+            x[k] = (cbytes[k] == 16 && p.m.aligned) ? ld16_stream(p.m.in + 16ull * g) : load_bytes(p.m.in + 16ull * g, cbytes[k]);
         } else {                                              // a10: BE64(8 a) || BE64(8 len)
-            const uint64_t abits = p.final_aad_len * 8, cbits = p.final_len * 8;
+            const uint64_t abits = p.m.final_aad_len * 8, cbits = p.m.final_len * 8;
             x[k] = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits),
                               bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
         }
     }
 
-    fill_aes_tables<SMALL_THREADS>(sm, p.tab.te0);
+    fill_aes_tables<SMALL_THREADS>(sm, p.te0, t);
     __syncthreads();
 
     // a3: E_K(J0), J0 = IV || 0^31 || 1, by the last warp; it reaches thread 0 through shared memory
@@ -79,8 +81,8 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
             const uint32_t g = i - n_aad;
             const uint4 ks = aes_encrypt_block<NR>(p.rk, sm, lane4, make_uint4(p.iv[0], p.iv[1], p.iv[2], bswap32(g + 2u)));
             const uint4 y = xor4(x[k], ks);
-            if (cbytes[k] == 16 && p.aligned) st16_stream(p.out + 16ull * g, y);
-            else store_bytes(p.out + 16ull * g, y, cbytes[k]);
+            if (cbytes[k] == 16 && p.m.aligned) st16_stream(p.m.out + 16ull * g, y);
+            else store_bytes(p.m.out + 16ull * g, y, cbytes[k]);
             if (MODE == MODE_ENCRYPT) X = keep_bytes(y, cbytes[k]);
         }
         acc = xor4(acc, gf_mul_mem(X, w[k]));                 // a7: X_i . H^(N - i)
@@ -102,18 +104,12 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
 template <int NR, int MODE>
 static cudaError_t launch_small_one(const GcmParams &p, cudaStream_t s)
 {
-    static bool configured[64] = {false};
-    auto kern = gcm_small_kernel<NR, MODE>;
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
+    static std::atomic<bool> configured[GCM_MAX_DEVICES];
+    const void *kern = (const void *)gcm_small_kernel<NR, MODE>;
+    cudaError_t e = ensure_smem_attr(kern, configured, SMALL_SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64 || !configured[dev]) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) configured[dev] = true;
-    }
-    kern<<<1, SMALL_THREADS, SMALL_SMEM_BYTES, s>>>(p);
-    return cudaGetLastError();
+    void *args[] = {(void *)&p};
+    return launch_with_pdl(kern, dim3(1), dim3(SMALL_THREADS), SMALL_SMEM_BYTES, s, args);
 }
 
 cudaError_t launch_small(int nr, int mode, const GcmParams &p, cudaStream_t s)

@@ -276,7 +276,7 @@ int ensure_key(gfc_context *c, int which, const uint8_t *key, int key_bits)
     if (c->g[which] && c->key_bits[which] == key_bits && memcmp(c->key[which], key, key_bits / 8) == 0) return GCM_OK;
     if (c->g[which]) gcm_destroy(c->g[which]);
     c->g[which] = nullptr;
-    int rc = gcm_init(&c->g[which], key, key_bits);
+    int rc = gcm_init_on_device(&c->g[which], key, key_bits, c->device);
     if (rc != GCM_OK) return rc;
     memcpy(c->key[which], key, key_bits / 8);
     c->key_bits[which] = key_bits;
@@ -400,7 +400,12 @@ extern "C" int gfc_context_create(gfc_context **out, uint64_t max_header_bytes, 
     c->max_data = max_data_bytes;
     // container = envelope header (hex ENCHDR: 160 card bytes per 67 hex characters) + BINTABLE header + payload
     c->out_cap = 5 * c->max_header + c->max_data + 16 * kBlock;
-    cudaError_t e = cudaGetDevice(&c->device);
+    // the library's one notion of "the device": gcm_set_device's choice, else the caller's current device
+    cudaError_t e = cudaSuccess;
+    int rc_dev = gcm_default_device(&c->device);
+    if (rc_dev != GCM_OK) { delete c; return rc_dev; }
+    DeviceGuard guard(c->device);
+    e = guard.err;
     do {
         if (e != cudaSuccess) break;
         if ((e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device)) != cudaSuccess) break;
@@ -428,6 +433,7 @@ extern "C" int gfc_context_create(gfc_context **out, uint64_t max_header_bytes, 
 extern "C" void gfc_context_destroy(gfc_context *c)
 {
     if (!c) return;
+    DeviceGuard guard(c->device);
     if (c->streamH) cudaStreamSynchronize(c->streamH);
     if (c->streamD) cudaStreamSynchronize(c->streamD);
     for (int i = 0; i < 2; i++) {
@@ -461,7 +467,8 @@ extern "C" int gfc_encrypt_frame(gfc_context *c, const uint8_t *fits, uint64_t f
         return fail(res, GFC_ERR_FORMAT, "not a FITS file: primary header without END / BITPIX / NAXIS");
     const uint64_t hlen = hd.length, n = fits_len - hlen;
     if (hlen > c->max_header || n > c->max_data) return fail(res, GFC_ERR_CAPACITY, "file larger than the context was created for");
-    CUF(cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    CUF(guard.err);
     int rc = ensure_key(c, 0, key_h, key_bits);
     if (rc == GCM_OK) rc = ensure_key(c, 1, key_d, key_bits);
     if (rc != GCM_OK) return fail(res, rc, "key setup failed");
@@ -557,7 +564,8 @@ extern "C" int gfc_decrypt_frame(gfc_context *c, const uint8_t *ctr, uint64_t le
     const std::string fb = minimal_header(o);
     const uint64_t room = hlen > fb.size() ? hlen : fb.size();     // the payload lands behind the larger header
     if (room + n > c->out_cap) return fail(res, GFC_ERR_CAPACITY, "result larger than the result buffer");
-    CUF(cudaSetDevice(c->device));
+    DeviceGuard guard(c->device);
+    CUF(guard.err);
 
     // ---- streamH: ENCHDR (L214); no Header Key -> nothing to do, the fallback header is used (L241)
     bool header_sent = false;

@@ -11,7 +11,8 @@ import ctypes
 import os
 from typing import Iterable, List, Optional, Sequence, Tuple
 
-GCM_OK, GCM_ERR_AUTH, GCM_ERR_ARG, GCM_ERR_LEN, GCM_ERR_CUDA, GCM_ERR_NOMEM = 0, 1, -1, -2, -3, -4
+GCM_OK, GCM_ERR_AUTH, GCM_ERR_ARG, GCM_ERR_LEN, GCM_ERR_CUDA, GCM_ERR_NOMEM, GCM_ERR_BUSY = 0, 1, -1, -2, -3, -4, -5
+GCM_PHASE_SLOTS = 8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libb200gcm.so")
@@ -20,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "gcm_version", "gcm_set_device", "gcm_last_cuda_error", "gcm_last_cuda_error_string",
     "gcm_init", "gcm_destroy", "gcm_set_geometry", "gcm_get_geometry", "gcm_get_hash_subkey",
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
-    "gcm_encrypt_host", "gcm_decrypt_verify_host",
+    "gcm_encrypt_host", "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
     "gcm_measure_pipe_rates",
 ]
@@ -82,6 +83,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_ghash_async.argtypes = [vp, vp, u64, vp, u64, vp, vp]
     L.gcm_encrypt_host.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
     L.gcm_decrypt_verify_host.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
+    L.gcm_decrypt_verify_host_strict.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
+    L.gcm_set_phase_stamps.argtypes = [vp, vp]
     L.gcm_encrypt_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_batch_release.argtypes = []
@@ -290,6 +293,26 @@ def gcm_decrypt_verify_host(ctx: int, iv: bytes, h_aad, h_ct, h_pt, tag: bytes, 
                 "gcm_decrypt_verify_host", ok=(GCM_OK, GCM_ERR_AUTH))
     del ka, kp, kc
     return rc
+
+
+def gcm_decrypt_verify_host_strict(ctx: int, iv: bytes, h_aad, h_ct, h_pt, tag: bytes, stream=None) -> int:
+    """Verify-then-release: h_pt is written only after the tag has been verified (two passes over h_ct)."""
+    iv, tag = _iv(iv), _tag(tag)
+    a_ptr, a_len, ka = _host(h_aad)
+    c_ptr, c_len, kc = _host(h_ct)
+    p_ptr, p_len, kp = _host(h_pt, writable=True)
+    if c_len != p_len:
+        raise ValueError("ct and pt sizes differ")
+    rc = _check(_L.gcm_decrypt_verify_host_strict(ctx, iv, a_ptr, a_len, c_ptr, c_len, p_ptr, tag, _stream(stream)),
+                "gcm_decrypt_verify_host_strict", ok=(GCM_OK, GCM_ERR_AUTH))
+    del ka, kp, kc
+    return rc
+
+
+def gcm_set_phase_stamps(ctx: int, d_stamps) -> None:
+    """Diagnostics: d_stamps = device buffer of GCM_PHASE_SLOTS x grid uint64 (or None to switch it off)."""
+    ptr, n = _dev(d_stamps)
+    _check(_L.gcm_set_phase_stamps(ctx, ptr), "gcm_set_phase_stamps")
 
 
 def gcm_ghash_async(ctx: int, aad, c, d_out, stream=None) -> None:
