@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-mib", type=float, default=384.0)
     ap.add_argument("--workload", default="c5",
-                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum", "phases"],
+                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum", "phases", "sizes"],
                     help="c5 = the headline (default); the others are the supplementary measurements of DESIGN.md section 10")
     return ap.parse_args()
 
@@ -125,17 +125,70 @@ def measured_peaks() -> dict:
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
 
 
-def pipe_bound_gbs(nr: int, sm_count: int, sm_mhz: float, mode: str = "enc") -> dict:
-    """Shared-memory-pipe bound of the method.  Per 16-byte block the path needs
-    16*nr conflict-free 4-byte AES table reads minus the ones that do not depend on the low counter
-    byte (12 round-1 reads of the constant IV columns, hoisted per thread; 3 round-1 + 12 round-2
-    reads cached per lane and refreshed every 8th block: -27 + 15/8), plus 16 16-byte GHASH table
-    reads = 64 bank-lanes; an SM serves 32 bank-lanes (one 128-byte wavefront) per cycle.
-    mode "ghash": the GHASH table reads alone."""
-    lanes = 64.0 if mode == "ghash" else 16 * nr - 27 + 15.0 / 8.0 + 64
-    cycles = lanes / 32.0
-    return {"lanes_per_block": lanes, "cycles_per_block_per_sm": cycles,
-            "gbs": sm_count * sm_mhz * 1e6 * 16.0 / cycles / 1e9}
+MIX_FILE = os.path.join(ROOT, "profiles", "sass_mix_r02.json")
+
+
+def load_mix(key: str) -> dict:
+    """Executed instruction mix of a kernel's row loop per warp-row (32 blocks), written by
+    `python -m paper_2602_23067_b200.profile_tools mix` from the ncu source page of the shipped kernel
+    (profiles/README_r02.md has the commands).  The roofline is built from it, not from a typed-in formula."""
+    try:
+        return json.load(open(MIX_FILE))[key]
+    except Exception as e:
+        raise SystemExit("bench.py: %s has no usable entry %r (%s): capture it as profiles/README_r02.md says; the roofline "
+                         "is derived from the shipped binary's executed mix and is not guessed" % (MIX_FILE, key, e))
+
+
+def pipe_bound_gbs(key: str, nr: int, sm_count: int, sm_mhz: float, rates: dict = None, ghash_only: bool = False) -> dict:
+    """Shared-memory-pipe (LSU data pipe) bound.  An SM retires one 128-byte shared-memory wavefront per cycle: a
+    conflict-free LDS.32 of a warp is one wavefront, an LDS.64 two, an LDS.128 four; a warp-row is 32 blocks, one per
+    lane, so wavefronts per warp-row = bank-lanes per block and cycles per block per SM = that / 32.
+      lanes            from the kernel's own executed mix (load_mix): the binding roofline north_star defines
+      with measured rates   the same counts against gcm_measure_pipe_rates' LDS.32 / LDS.128 rates of this device
+      yardsticks       kernel-independent ('so a bloated kernel cannot flatter itself'): the plain
+                       table design (16 T-table reads per round + a 16-lookup 8-bit Shoup multiply: 16 nr + 64 lanes)
+                       and the AES table reads alone with every hoistable read hoisted (16 nr - 27 + 15/8)."""
+    e = load_mix(key)["per_warp_row"]
+    lanes = e["lds32"] + 2.0 * e["lds64"] + 4.0 * e["lds128"]
+    glob = 4.0 * (e["ldg128"] + e["stg128"])
+    scale = sm_count * sm_mhz * 1e6 * 16.0 / 1e9
+    out = {"mix": key, "lanes_per_block": lanes, "global_lanes_per_block": glob, "cycles_per_block_per_sm": lanes / 32.0,
+           "gbs": scale / (lanes / 32.0), "gbs_with_global_wavefronts": scale / ((lanes + glob) / 32.0),
+           "counts_per_block": {k: round(e[k], 3) for k in ("lds32", "lds64", "lds128", "ldg128", "stg128")},
+           "alu_thread_instructions_per_block": e["by_pipe_warp_instructions"].get("alu"),
+           "fma_thread_instructions_per_block": e["by_pipe_warp_instructions"].get("fma"),
+           "thread_instructions_per_block": e["warp_instructions"]}
+    if rates and rates.get("lds32") and rates.get("lds128"):
+        cyc = e["lds32"] / rates["lds32"] + 2.0 * e["lds64"] / (2.0 * rates["lds128"]) + e["lds128"] / rates["lds128"]
+        out["gbs_measured_rates"] = scale / cyc
+    naive = 64.0 if ghash_only else 16.0 * nr + 64.0
+    out["yardsticks"] = {"plain_table_design_lanes": naive, "plain_table_design_gbs": scale / (naive / 32.0)}
+    if not ghash_only:
+        floor = 16.0 * nr - 27.0 + 15.0 / 8.0
+        out["yardsticks"].update(aes_reads_only_lanes=floor, aes_reads_only_gbs=scale / (floor / 32.0))
+    return out
+
+
+def roofline_dict(pb: dict, achieved: float, peaks: dict, hbm_bytes_per_byte: int) -> dict:
+    """The contract's roofline object for a kernel bound by the shared-memory data pipe."""
+    hbm_peak = float(peaks["hbm_gbs"])
+    y = pb["yardsticks"]
+    r = {"bound": "alu", "unit_pipe": "lsu_shared",
+         "pipe": "shared-memory data pipe (LSU): %.1f bank-lanes per 16-byte block from the kernel's executed mix "
+                 "(%s), 32 per SM-cycle" % (pb["lanes_per_block"], pb["mix"]),
+         "achieved": achieved, "peak": pb["gbs"], "unit": UNIT, "frac": achieved / pb["gbs"],
+         "frac_with_global_wavefronts": achieved / pb["gbs_with_global_wavefronts"],
+         "counts_per_block": pb["counts_per_block"],
+         "yardsticks": {k: (round(v, 1) if isinstance(v, float) else v) for k, v in y.items()},
+         "frac_of_plain_table_design": achieved / y["plain_table_design_gbs"],
+         "hbm": {"achieved": hbm_bytes_per_byte * achieved, "peak": hbm_peak, "unit": "GB/s",
+                 "frac": hbm_bytes_per_byte * achieved / hbm_peak, "of": peaks["_source"]}}
+    if "aes_reads_only_gbs" in y:
+        r["frac_of_aes_reads_only_floor"] = achieved / y["aes_reads_only_gbs"]
+    if "gbs_measured_rates" in pb:
+        r["peak_measured_rates"] = pb["gbs_measured_rates"]
+        r["frac_measured_rates"] = achieved / pb["gbs_measured_rates"]
+    return r
 
 
 def traffic_per_launch(payload_bytes: int):
@@ -197,6 +250,54 @@ def cpu_context(key, iv):
     except Exception as e:                      # context only
         out["openssl"] = "unavailable: %s" % type(e).__name__
     return out
+
+
+def pcie_duplex_gbs(nbytes: int = 1 << 30, reps: int = 3) -> dict:
+    """What the host link gives: one pinned H2D copy and one pinned D2H copy of `nbytes` each, alone and both at once
+    on two streams (the e2e path moves the message both ways at the same time).  GB/s per direction, best of reps."""
+    import torch
+    h_a = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    h_b = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d_a = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    d_b = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run(h2d: bool, d2h: bool) -> float:
+        best = 1e30
+        for _ in range(reps + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            if h2d:
+                with torch.cuda.stream(s1):
+                    d_a.copy_(h_a, non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s2):
+                    h_b.copy_(d_b, non_blocking=True)
+            torch.cuda.synchronize()
+            best = min(best, time.perf_counter() - t0)
+        return nbytes / best / 1e9
+
+    out = {"h2d_alone": run(True, False), "d2h_alone": run(False, True), "per_direction_duplex": run(True, True),
+           "bytes": nbytes, "how": "torch copy_ of pinned buffers, one cudaMemcpyAsync per direction, host wall clock, best of %d" % reps}
+    del h_a, h_b, d_a, d_b
+    return out
+
+
+def oracle_batch_gbs(msgs, what: str) -> dict:
+    """cpu_baseline of the batched configs: the oracle as it stands, one whole message per task, tasks spread over the
+    host cores (independent messages: SURVEY.md 8(d))."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import oracle as O
+    cores = os.cpu_count() or 1
+    O.lib()
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(cores) as ex:
+        tags = list(ex.map(lambda m: O.gcm_encrypt(m.key, m.iv, m.aad, m.payload)[1], msgs))
+    dt = time.perf_counter() - t0
+    nbytes = sum(m.payload.size for m in msgs)
+    assert len(tags) == len(msgs)
+    return {"value": nbytes / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+            "sample": "%s: %d messages, %d bytes, one message per task over %d threads" % (what, len(msgs), nbytes, cores)}
 
 
 def run_reference(args):
@@ -326,6 +427,12 @@ def run_ours(args):
                "h2d_bytes_per_step": n + int(m.aad.size), "d2h_bytes_per_step": n + 16,
                "steps": args.e2e_steps, "how": "gcm_encrypt_host: pinned host in/out, chunked H2D -> fused kernel -> D2H"}
         del h_pt, h_ct
+        if rank == 0:
+            # the bound of this leg: the message crosses the host link once in each direction, at the same time
+            link = pcie_duplex_gbs(min(n, 1 << 30))
+            e2e["pcie_peak"] = link["per_direction_duplex"]
+            e2e["frac"] = e2e["value"] / world / link["per_direction_duplex"]
+            e2e["pcie"] = link
 
     G.gcm_destroy(ctx)
     if rank != 0:
@@ -336,24 +443,21 @@ def run_ours(args):
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     kernel_ms = statistics.mean(per)
     achieved = n / (kernel_ms * 1e-3) / 1e9
-    pb = pipe_bound_gbs(14, sm_count, float(peaks.get("sm_max_mhz", 1965.0)))
-    hbm_peak = float(peaks["hbm_gbs"])
-    roofline = {
-        "bound": "alu", "pipe": "shared-memory wavefronts (LSU): %.1f bank-lanes per 16-byte block, 32 per SM-cycle" % pb["lanes_per_block"],
-        "achieved": achieved, "peak": pb["gbs"], "unit": UNIT, "frac": achieved / pb["gbs"],
-        "peak_source": "derived (DESIGN.md section 6): %d SMs x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s) x 16 B / %.3f cycles"
-                       % (sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks["_source"], pb["cycles_per_block_per_sm"]),
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    pb = pipe_bound_gbs("fused_aes256_enc", 14, sm_count, sm_mhz, rates)
+    roofline = roofline_dict(pb, achieved, peaks, 2)
+    roofline.update({
+        "peak_source": "derived (DESIGN.md section 6): %d SMs x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s) x 16 B / %.3f cycles; "
+                       "lanes from %s" % (sm_count, sm_mhz, peaks["_source"], pb["cycles_per_block_per_sm"], os.path.relpath(MIX_FILE, ROOT)),
         "traffic": traffic_per_launch(n),
         "algorithmic_bytes_per_launch": 2 * n,
-        "hbm": {"achieved": 2 * achieved, "peak": hbm_peak, "unit": "GB/s", "frac": 2 * achieved / hbm_peak,
-                "of": peaks["_source"]},
         "rates": {"unit": "thread-operations per SM-cycle, measured by gcm_measure_pipe_rates on this device",
                   **{k: round(v, 2) for k, v in rates.items()}},
         "kernel": "gcm_fused_kernel<14, ENCRYPT, 512>", "kernel_ms_mean": kernel_ms,
         "kernel_ms_median": statistics.median(per),
-    }
+    })
     if clocks.get("sm_mhz"):
-        roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs(14, sm_count, clocks["sm_mhz"])["gbs"]
+        roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs("fused_aes256_enc", 14, sm_count, clocks["sm_mhz"])["gbs"]
 
     cpu = None
     verified = 0
@@ -462,13 +566,12 @@ def run_extra(args):
             assert int(d_status.item()) == 0 and torch.equal(back[:1 << 20], pt[:1 << 20])
         G.gcm_destroy(ctx)
         gbs = steps * n / (total_ms * 1e-3) / 1e9
-        pb = pipe_bound_gbs(nr, sm_count, sm_mhz, mode)
+        key_mix = {"c5-decrypt": "fused_aes256_dec", "c5-ghash": "fused_ghash", "c5-aes128": "fused_aes128_enc", "c2": "fused_aes256_enc"}[w]
+        pb = pipe_bound_gbs(key_mix, nr, sm_count, sm_mhz, G.gcm_measure_pipe_rates(), ghash_only=(mode == "ghash"))
         line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
                     config={"workload": "%s: %s, %d-byte message, 2880-byte AAD" % (w, what, n), "payload_bytes": n},
                     gpu_launches=launches * steps, clocks=clocks,
-                    roofline={"bound": "alu", "pipe": "shared-memory wavefronts (LSU): %.1f bank-lanes per block" % pb["lanes_per_block"],
-                              "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"],
-                              "hbm_frac": (1 if mode == "ghash" else 2) * gbs / float(peaks["hbm_gbs"])},
+                    roofline=roofline_dict(pb, gbs, peaks, 1 if mode == "ghash" else 2),
                     ms_per_step_median=statistics.median(per))
     elif w == "c3":
         msgs = workloads.config_c3()
@@ -481,13 +584,15 @@ def run_extra(args):
         total_ms, per, clocks = timed(lambda: G.gcm_encrypt_batch(batch, stream))
         G.gcm_batch_release()
         gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
-        pb = pipe_bound_gbs(14, sm_count, sm_mhz)
+        pb = pipe_bound_gbs("multi_aes256_enc", 14, sm_count, sm_mhz, G.gcm_measure_pipe_rates())
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"] = oracle_batch_gbs(msgs, "C3")
         line.update(metric="AES-256-GCM batched encrypt GB/s (C3: 16 FITS images of 64 MiB)", value=gbs,
                     ms_per_step=total_ms / steps, gpu_launches=steps, clocks=clocks,
                     config={"workload": "c3: gcm_encrypt_batch, 16 x 67,109,760-byte FITS-shaped images, one AES-256 key, 16 IVs, "
                                         "2880-byte header AAD each; synchronous call (descriptor upload, ONE multi-message launch, tag download inside)",
                             "payload_bytes": nbytes},
-                    roofline={"bound": "alu", "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"]},
+                    roofline=roofline_dict(pb, gbs, peaks, 2),
                     ms_per_step_median=statistics.median(per))
     elif w == "c4":
         msgs = workloads.config_c4()
@@ -515,7 +620,28 @@ def run_extra(args):
         total_ms, per, clocks = timed(step)
         G.gcm_batch_release()
         gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
-        pb = pipe_bound_gbs(10, sm_count, sm_mhz)
+        pb = pipe_bound_gbs("batch_aes128_enc", 10, sm_count, sm_mhz, G.gcm_measure_pipe_rates())
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"] = oracle_batch_gbs(msgs, "C4")
+        # C4's latency report: one 1 KiB and one 64 KiB message through the synchronous non-batched call
+        lat = {}
+        mk = workloads.config_c1(payload_bytes=0)
+        lctx = G.gcm_init(mk.key)
+        l_aad = torch.from_numpy(mk.aad).cuda()
+        for ln in (1024, 65536):
+            l_pt = rand_bytes(ln, 7 + ln)
+            l_ct = torch.empty_like(l_pt)
+            for _ in range(50):
+                G.gcm_encrypt(lctx, mk.iv, l_aad, l_pt, l_ct, stream)
+            ts = []
+            for _ in range(1000):
+                t0 = time.perf_counter()
+                G.gcm_encrypt(lctx, mk.iv, l_aad, l_pt, l_ct, stream)
+                ts.append((time.perf_counter() - t0) * 1e6)
+            ts.sort()
+            lat["%d_bytes" % ln] = {"p50_us": ts[len(ts) // 2], "p99_us": ts[int(len(ts) * 0.99)]}
+        G.gcm_destroy(lctx)
+        line["single_message_latency"] = lat
         line.update(metric="AES-128-GCM batched encrypt GB/s (C4: 10,000 messages of 1 B..64 KiB)", value=gbs,
                     ms_per_step=total_ms / steps, gpu_launches=2 * steps, clocks=clocks,
                     messages_per_s=steps * len(msgs) / (total_ms * 1e-3),
@@ -523,9 +649,10 @@ def run_extra(args):
                                         "own key and IV each, payloads packed at 16-byte-aligned offsets; synchronous call "
                                         "(descriptor upload, one persistent warp-per-message kernel, tag download inside)",
                             "payload_bytes": nbytes, "messages": len(msgs)},
-                    roofline={"bound": "alu", "achieved": gbs, "peak": pb["gbs"], "unit": UNIT, "frac": gbs / pb["gbs"],
-                              "note": "peak is the large-message bound of the 8-bit-table kernel; the per-message key schedule, "
-                                      "H ladder and 4-bit table build of this kernel are not in it"},
+                    roofline=dict(roofline_dict(pb, gbs, peaks, 2),
+                                  note="the kernel's own mix: 4-bit GHASH table (32 LDS.128 per block) and per-message key "
+                                       "schedule, H ladder, table build and tree; achieved is the synchronous C call, host "
+                                       "marshalling and transfers included"),
                     ms_per_step_median=statistics.median(per))
     elif w == "datasum":
         # DATASUM reduction kernel (FITS checksum of the encrypted payload): HBM-bound, 1 byte read per byte
@@ -581,6 +708,43 @@ def run_extra(args):
                     gpu_launches=None, frames=out,
                     config={"workload": "frame: gfc_encrypt_frame / gfc_decrypt_frame (AES-256, dual key) on a 256x256 and a 4096x4096 float32 "
                                         "FITS file in pinned host memory; H2D and D2H inside the timed region (PCIe-bound)"})
+    elif w == "sizes":
+        # Throughput by message size around the paper's FITS files (17 / 201 / 577 MB, PAPER.md Table A.7): trains of
+        # launches back to back on one stream, one event pair around the whole train (an event between two launches
+        # costs about 5 us and switches programmatic dependent launch off).
+        m = workloads.config_c2(payload_bytes=0)
+        ctx = G.gcm_init(m.key)
+        aad = torch.from_numpy(m.aad).cuda()
+        d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        pb = pipe_bound_gbs("fused_aes256_enc", 14, sm_count, sm_mhz)
+        out = {}
+        for mib in (1, 4, 16, 64, 256, 1024):
+            n = mib << 20
+            pt = rand_bytes(n, 200 + mib)
+            ct = torch.empty_like(pt)
+            reps = max(steps, 20 if mib >= 256 else 200)
+            best = None
+            for _ in range(3):
+                for _ in range(warm):
+                    G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(reps):
+                    G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                us = e0.elapsed_time(e1) * 1e3 / reps
+                best = us if best is None else min(best, us)
+            out["%d_MiB" % mib] = {"us_per_launch": best, "GBps": n / best / 1e3, "frac_of_pipe_bound": n / best / 1e3 / pb["gbs"]}
+            del pt, ct
+        G.gcm_destroy(ctx)
+        line.update(metric="AES-256-GCM encrypt GB/s by message size (device-timed trains of launches)",
+                    value=out["16_MiB"]["GBps"], ms_per_step=out["16_MiB"]["us_per_launch"] / 1e3, gpu_launches=None, sizes=out,
+                    roofline={"bound": "alu", "unit_pipe": "lsu_shared", "peak": pb["gbs"], "unit": UNIT,
+                              "achieved": out["16_MiB"]["GBps"], "frac": out["16_MiB"]["frac_of_pipe_bound"]},
+                    config={"workload": "sizes: AES-256-GCM encrypt of 1 MiB .. 1 GiB device-resident messages, 2880-byte AAD, launches "
+                                        "back to back; pdl=%s; messages of 16 MiB and less fit in the 126 MB L2 (in + out)"
+                                        % ("off" if os.environ.get("GCM_NO_PDL") else "on")})
     elif w == "phases":
         # Where the fixed cost of a launch goes: the fused kernel's own %globaltimer stamps
         # (gcm_set_phase_stamps) for message sizes around the paper's FITS files, launches back to back on one stream.

@@ -192,15 +192,17 @@ __device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *r
 }
 
 // order[j]: message index of the j-th ticket (longest first); next: ticket counter.
+struct Te0Param { uint32_t w[256]; };      // the round table T0 by value: constant bank, no global load at kernel start
+
 template <int NR, int MODE>
 __global__ void __launch_bounds__(BATCH_THREADS, 1)
 gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *order, uint32_t n,
-                 unsigned *next, const uint32_t *te0)
+                 unsigned *next, const __grid_constant__ Te0Param te0)
 {
     extern __shared__ __align__(1024) uint8_t sm[];
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t warp = __shfl_sync(0xFFFFFFFFu, threadIdx.x >> 5, 0);
-    fill_aes_tables<BATCH_THREADS>(sm, te0, threadIdx.x);
+    fill_aes_tables<BATCH_THREADS>(sm, te0.w, threadIdx.x);
     __syncthreads();
     uint8_t *tab = sm + BATCH_TAB_OFF + warp * BATCH_TAB_BYTES;
     uint4 *hp = reinterpret_cast<uint4 *>(sm + BATCH_HP_OFF + warp * BATCH_HP_BYTES);
@@ -218,7 +220,7 @@ gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *o
 
 template <int NR, int MODE>
 static cudaError_t launch_batch(int blocks, const BatchDesc *descs, BatchResult *results, const uint32_t *order,
-                                uint32_t n, unsigned *next, const uint32_t *te0, cudaStream_t s)
+                                uint32_t n, unsigned *next, const Te0Param &te0, cudaStream_t s)
 {
     static std::atomic<bool> configured[GCM_MAX_DEVICES];
     auto kern = gcm_batch_kernel<NR, MODE>;
@@ -245,6 +247,7 @@ struct BatchState {
     uint32_t *h_order = nullptr, *d_order = nullptr;
     unsigned *d_next = nullptr;      // [2]
     uint32_t *d_te0 = nullptr;
+    Te0Param h_te0;                  // host copy of the round table (made on the device by gcm_te0_kernel)
     // staging of the large-message path (gcm_multi.cu): descriptors, chunks, per-warp chunk ranges,
     // accumulators + tickets; one pinned block and one device block, grown on demand
     uint8_t *h_multi = nullptr, *d_multi = nullptr;
@@ -315,7 +318,7 @@ int ensure_staging_locked(uint32_t n)
             if ((e = cudaMalloc((void **)&g.d_te0, 256 * sizeof(uint32_t))) != cudaSuccess) break;
             launch_te0(g.d_te0, 0);
             if ((e = cudaGetLastError()) != cudaSuccess) break;
-            if ((e = cudaDeviceSynchronize()) != cudaSuccess) break;
+            if ((e = cudaMemcpy(g.h_te0.w, g.d_te0, sizeof(g.h_te0.w), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         } while (0);
         if (e != cudaSuccess) {
             int rc = gcm_cuda_fail(e);
@@ -482,6 +485,7 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
 
     int first_err = GCM_OK;
     std::vector<uint32_t> small[2], large;                  // small[0]: AES-128, small[1]: AES-256
+    small[0].reserve(n); small[1].reserve(n);
     for (uint32_t i = 0; i < n; i++) {
         gcm_msg &m = msgs[i];
         m.status = check_msg(m);
@@ -515,16 +519,17 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     CUB(cudaMemcpyAsync(g.d_desc, g.h_desc, (size_t)n * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
     if (pos) CUB(cudaMemcpyAsync(g.d_order, g.h_order, (size_t)pos * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
     CUB(cudaMemsetAsync(g.d_next, 0, 2 * sizeof(unsigned), s));
-    CUB(cudaMemsetAsync(g.d_res, 0, (size_t)n * sizeof(BatchResult), s));
+    // verdicts fail closed: a result slot that no kernel writes reads "refused", never a stale 0 of an earlier call
+    if (decrypt) CUB(cudaMemsetAsync(g.d_res, 0xFF, (size_t)n * sizeof(BatchResult), s));
     for (int k = 0; k < 2; k++) {
         if (!count[k]) continue;
         const uint32_t want = (count[k] + BATCH_WARPS - 1) / BATCH_WARPS;
         const int blocks = (int)std::min<uint32_t>(want, (uint32_t)g.sm_count);
         cudaError_t e;
-        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s)
-                                : launch_batch<10, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s);
-        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s)
-                                : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.d_te0, s);
+        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s)
+                                : launch_batch<10, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s);
+        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s)
+                                : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s);
         if (e != cudaSuccess) return gcm_cuda_fail(e);
     }
     rc = run_large_locked(msgs, large, decrypt, s, &first_err);

@@ -338,7 +338,10 @@ struct MulK8 {                 // 8-bit Shoup table of K in shared memory at KTA
 // RK:  indexable round keys.  MUL: y -> y . K.  Returns the lane's running value Y (a7) after its last block.
 // The same code serves the single-message kernel (gcm_fused.cu), the many-large-messages kernel (gcm_multi.cu)
 // and the warp-per-message kernel (gcm_batch.cu).
-template <int NR, int MODE, class MSG, class RK, class MUL>
+// DEPTH: rows of payload a lane keeps in flight ahead of the one it works on.  One row (512 B per warp, 8 KB per
+// SM) covers the 1 TB/s the AES modes read; GHASH-only reads twice as fast and needs more bytes in flight to
+// cover the HBM latency (Little's law: 2 TB/s x 0.8 us = 11 KB per SM).
+template <int NR, int MODE, int DEPTH = 1, class MSG, class RK, class MUL>
 __device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint8_t *sm, uint32_t lane,
                                           const CtrConst &cc, uint32_t r0, uint32_t r1, const MUL &mul)
 {
@@ -347,18 +350,43 @@ __device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint
     uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
     bool have_pre = false;
+    const uint32_t first_fast = r0 > m.fast_lo() ? r0 : m.fast_lo();      // first fast row of this run (if any)
+    const uint32_t lim = r1 < m.fast_hi() ? r1 : m.fast_hi();             // fast rows of this run end here
     for (uint32_t row = r0; row < r1; row++) {
         const uint64_t v = 32ull * row + lane;          // virtual block index
         const bool fast = row >= m.fast_lo() && row < m.fast_hi();
+        if (MODE == MODE_GHASH && DEPTH > 1 && fast && row == first_fast) {
+            // GHASH only: all fast rows of the run in a DEPTH-deep software pipeline, unrolled DEPTH times so that
+            // the slots keep their registers (no shifting); then on with the (slow) rows behind them
+            const uint8_t *src = m.in() + 16 * (v - m.base());
+            const uint32_t n = lim - row;
+            uint4 buf[DEPTH];
+#pragma unroll
+            for (int k = 0; k < DEPTH; k++) buf[k] = (uint32_t)k < n ? ld16_stream(src + 512 * k) : make_uint4(0, 0, 0, 0);
+            uint32_t i = 0;
+            for (; i + DEPTH <= n; i += DEPTH) {
+#pragma unroll
+                for (int k = 0; k < DEPTH; k++) {
+                    const uint4 xk = buf[k];
+                    if (i + DEPTH + k < n) buf[k] = ld16_stream(src + 512ull * (i + DEPTH + k));
+                    Y = xor4(mul(Y), xk);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < DEPTH; k++)
+                if (i + k < n) Y = xor4(mul(Y), buf[k]);
+            row = lim - 1;
+            continue;
+        }
         uint4 x = make_uint4(0, 0, 0, 0);
         uint32_t cbytes = 0;                            // payload bytes in this block (0: pad / AAD / length block / beyond the end)
         uint64_t g = 0;                                 // payload block index
         bool valid = true;
         if (fast) {
             g = v - m.base();
-            x = have_pre ? pre : ld16_stream(m.in() + 16 * g);
             cbytes = 16;
-            have_pre = row + 1 < r1 && row + 1 < m.fast_hi();
+            x = have_pre ? pre : ld16_stream(m.in() + 16 * g);
+            have_pre = row + 1 < lim;
             if (have_pre) pre = ld16_stream(m.in() + 16 * g + 512);
         } else {
             have_pre = false;

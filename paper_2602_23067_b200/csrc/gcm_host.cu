@@ -11,6 +11,10 @@
 #include <cuda_runtime.h>
 #include <string.h>
 #include <new>
+#ifdef GCM_PIPE_DEBUG
+#include <chrono>
+#include <stdio.h>
+#endif
 
 #include "../../include/gcm.h"
 #include "gcm_common.cuh"
@@ -23,13 +27,13 @@
 #ifndef PIPE_SLOTS
 #define PIPE_SLOTS 3
 #endif
-#define PIPE_CHUNK_BYTES (64ull << 20)   /* staging buffer = largest chunk; multiple of 16 */
+#ifndef PIPE_CHUNK_BYTES
+#define PIPE_CHUNK_BYTES (64ull << 20)   /* staging buffer = largest chunk; multiple of PIPE_MIN_CHUNK_BYTES */
+#endif
 #ifndef PIPE_MIN_CHUNK_BYTES
-#define PIPE_MIN_CHUNK_BYTES (4ull << 20)
+#define PIPE_MIN_CHUNK_BYTES (2ull << 20)   /* first and last chunk: what the pipeline cannot overlap */
 #endif
-#ifndef PIPE_TARGET_CHUNKS
-#define PIPE_TARGET_CHUNKS 8
-#endif
+#define PIPE_MAX_CHUNKS ((uint32_t)((1ull << 36) / PIPE_CHUNK_BYTES) + 76)   /* 2^36 bytes in full chunks + the two ramps */
 
 struct HostPipe {
     cudaStream_t stream[PIPE_SLOTS];
@@ -39,7 +43,9 @@ struct HostPipe {
     uint8_t *d_aad;
     size_t aad_cap;
     uint4 *d_state;     // [2]: running GHASH state, ping-pong
-    uint4 *d_pows;      // [2]: H^(blocks of a full chunk), H^(blocks of the last chunk + the length block)
+    uint4 *d_pows;      // [PIPE_MAX_CHUNKS]: H^(GHASH blocks of chunk k)
+    uint64_t *d_exp;    // [PIPE_MAX_CHUNKS]: those block counts
+    uint64_t *h_exp;    // pinned staging of d_exp
 };
 
 #define CU(call)                                                                                   \
@@ -48,17 +54,52 @@ struct HostPipe {
         if (e__ != cudaSuccess) return gcm_cuda_fail(e__);                                         \
     } while (0)
 
-// out[i] = H^(e[i]) by square-and-multiply, one thread per exponent.
-__global__ void gcm_pow_kernel(const uint4 *h, uint64_t e0, uint64_t e1, uint4 *out)
+// out[k] = H^(e[k]), e[k] < 2^36, one thread per exponent: the product of four entries of the context's radix-512
+// digit tables hx[d*512 + j] = H^(j * 512^d) ("table of powers of the hash key").
+__global__ void gcm_chunk_pow_kernel(const uint4 *hx, const uint64_t *e, uint32_t n, uint4 *out)
 {
-    uint64_t e = threadIdx.x == 0 ? e0 : e1;
-    gf128 base = gf_from_mem(*h), r = gf_one();
-    while (e) {
-        if (e & 1) r = gf_mul(r, base);
-        base = gf_mul(base, base);
-        e >>= 1;
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const uint64_t d = e[k];
+    const uint32_t mask = (1u << HX_RADIX_BITS) - 1;
+    gf128 r = gf_from_mem(hx[(uint32_t)d & mask]);
+    for (uint32_t dig = 1; dig < HX_DIGITS; dig++) {
+        const uint32_t j = (uint32_t)(d >> (HX_RADIX_BITS * dig)) & mask;
+        if (j) r = gf_mul(r, gf_from_mem(hx[(dig << HX_RADIX_BITS) + j]));
     }
-    out[threadIdx.x] = gf_to_mem(r);
+    out[k] = gf_to_mem(r);
+}
+
+// Chunk lengths of a message of `len` bytes.  The first upload and the last download cannot overlap with anything,
+// so the plan starts and ends with PIPE_MIN_CHUNK_BYTES; chunks double up to the middle size (about len / 12, at
+// most PIPE_CHUNK_BYTES) and come down again by a factor of about 0.6, slowly enough that a chunk's download is
+// over before the upload two chunks later wants its slot (s_k <= s_(k+1) + s_(k+2)).  Every chunk but the last is
+// a multiple of PIPE_MIN_CHUNK_BYTES (so of 16); the last one takes the ragged end.
+static uint32_t plan_chunks(uint64_t len, uint64_t *plan)
+{
+    if (len == 0) { plan[0] = 0; return 1; }
+    const uint64_t U = PIPE_MIN_CHUNK_BYTES;
+    uint64_t mid = U;
+    while (mid * 2 <= len / 12 && mid * 2 <= PIPE_CHUNK_BYTES) mid *= 2;
+    uint64_t back[PIPE_MAX_CHUNKS];
+    uint32_t nf = 0, nb = 0;
+    const uint64_t last = ((len - 1) % U) + 1;
+    uint64_t rem = len - last;
+    back[nb++] = last;
+    uint64_t a = U, b = U;
+    while (rem > 0) {
+        uint64_t t = a < rem ? a : rem;
+        plan[nf++] = t; rem -= t;
+        a = a * 2 < mid ? a * 2 : mid;
+        if (rem > 0) {
+            t = b < rem ? b : rem;
+            back[nb++] = t; rem -= t;
+            b = (b * 8 / 5 + U - 1) / U * U;            // x 1.6, rounded up to the unit
+            if (b > mid) b = mid;
+        }
+    }
+    for (uint32_t i = nb; i-- > 0;) plan[nf++] = back[i];
+    return nf;
 }
 
 static void pipe_destroy(HostPipe *hp)
@@ -77,6 +118,8 @@ static void pipe_destroy(HostPipe *hp)
     if (hp->start) cudaEventDestroy(hp->start);
     if (hp->d_aad) cudaFree(hp->d_aad);
     if (hp->d_state) cudaFree(hp->d_state);
+    if (hp->d_exp) cudaFree(hp->d_exp);
+    if (hp->h_exp) cudaFreeHost(hp->h_exp);
     cudaGetLastError();
     delete hp;
 }
@@ -96,7 +139,9 @@ static int pipe_get(gcm_ctx *c, size_t aad_len)
             e = cudaMalloc((void **)&hp->d_stage[i], PIPE_CHUNK_BYTES);
         }
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->start, cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&hp->d_state, 4 * sizeof(uint4));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&hp->d_state, (2 + PIPE_MAX_CHUNKS) * sizeof(uint4));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&hp->d_exp, PIPE_MAX_CHUNKS * sizeof(uint64_t));
+        if (e == cudaSuccess) e = cudaHostAlloc((void **)&hp->h_exp, PIPE_MAX_CHUNKS * sizeof(uint64_t), cudaHostAllocDefault);
         if (e != cudaSuccess) {
             pipe_destroy(hp);
             return gcm_cuda_fail(e);
@@ -136,33 +181,35 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
     if (rc != GCM_OK) return rc;
     HostPipe *hp = c->pipe;
     cudaStream_t us = (cudaStream_t)user_stream;
+#ifdef GCM_PIPE_DEBUG
+    const auto t_begin = std::chrono::steady_clock::now();
+#endif
 
-    // about eight chunks per message so that H2D, kernel and D2H of neighbouring chunks overlap also for
-    // FITS-sized (tens of MiB) messages; 4 MiB at least (launch and table-fill cost), 64 MiB at most (staging)
-    uint64_t chunk = ((len / PIPE_TARGET_CHUNKS + (1ull << 20) - 1) >> 20) << 20;
-    if (chunk < PIPE_MIN_CHUNK_BYTES) chunk = PIPE_MIN_CHUNK_BYTES;
-    if (chunk > PIPE_CHUNK_BYTES) chunk = PIPE_CHUNK_BYTES;
-    const uint64_t n_chunks = len ? (len + chunk - 1) / chunk : 1;
-    const uint64_t last_len = len - (n_chunks - 1) * chunk;
+    // chunk plan: small chunks at both ends, PIPE_CHUNK_BYTES in the middle
+    uint64_t plan[PIPE_MAX_CHUNKS];
+    const uint32_t n_chunks = plan_chunks(len, plan);
     // work already queued on the caller's stream happens before ours
     CU(cudaEventRecord(hp->start, us));
     for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamWaitEvent(hp->stream[i], hp->start, 0));
     if (aad_len) CU(cudaMemcpyAsync(hp->d_aad, h_aad, aad_len, cudaMemcpyHostToDevice, hp->stream[0]));
     if (n_chunks > 1) {
-        // GHASH blocks per chunk: a middle chunk's payload blocks; the last chunk's plus the length block
-        gcm_pow_kernel<<<1, 2, 0, hp->stream[PIPE_SLOTS - 1]>>>(c->d_h, chunk / 16, (last_len + 15) / 16 + 1, hp->d_pows);
+        // chain_pow of chunk k: H^(GHASH blocks of chunk k) = its payload blocks, plus the length block in the last
+        cudaStream_t sp = hp->stream[PIPE_SLOTS - 1];
+        for (uint32_t k = 0; k < n_chunks; k++) hp->h_exp[k] = (plan[k] + 15) / 16 + (k == n_chunks - 1 ? 1 : 0);
+        CU(cudaMemcpyAsync(hp->d_exp, hp->h_exp, n_chunks * sizeof(uint64_t), cudaMemcpyHostToDevice, sp));
+        gcm_chunk_pow_kernel<<<(n_chunks + 63) / 64, 64, 0, sp>>>(c->d_hx, hp->d_exp, n_chunks, hp->d_pows);
         CU(cudaGetLastError());
-        CU(cudaEventRecord(hp->kernel_done[PIPE_SLOTS - 1], hp->stream[PIPE_SLOTS - 1]));
+        CU(cudaEventRecord(hp->kernel_done[PIPE_SLOTS - 1], sp));
     }
     // the verdict reads "refused" until the finisher of the last chunk has written it (fail closed)
     volatile int *verdict = (volatile int *)(c->h_pinned + 16);
     *verdict = GCM_STATUS_PENDING;
 
-    for (uint64_t k = 0; k < n_chunks; k++) {
+    uint64_t off = 0;
+    for (uint32_t k = 0; k < n_chunks; off += plan[k], k++) {
         const int slot = (int)(k % PIPE_SLOTS);
         cudaStream_t s = hp->stream[slot];
-        const uint64_t off = k * chunk;
-        const uint64_t clen = (k == n_chunks - 1) ? last_len : chunk;
+        const uint64_t clen = plan[k];
         const bool first = (k == 0), last = (k == n_chunks - 1);
         if (clen) CU(cudaMemcpyAsync(hp->d_stage[slot], (const uint8_t *)h_in + off, clen, cudaMemcpyHostToDevice, s));
         // kernels run in message order: chunk k needs chunk k-1's GHASH state (and the powers)
@@ -177,7 +224,7 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         if (rc != GCM_OK) return rc;
         if (!first) {
             p.chain_in = hp->d_state + ((k - 1) & 1);
-            p.chain_pow = hp->d_pows + (last ? 1 : 0);
+            p.chain_pow = hp->d_pows + k;
         }
         if (!last) p.chain_out = hp->d_state + (k & 1);
         if (mode == MODE_DECRYPT) memcpy(p.tag_expect, tag_io, 16);
@@ -191,7 +238,14 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         if (d_sum32 && mode == MODE_ENCRYPT) CU(launch_fits_sum32(hp->d_stage[slot], clen, d_sum32, c->sm_count, s));
         if (clen && mode != MODE_GHASH) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
     }
+#ifdef GCM_PIPE_DEBUG
+    const double t_enq = std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count();
+#endif
     for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamSynchronize(hp->stream[i]));
+#ifdef GCM_PIPE_DEBUG
+    fprintf(stderr, "pipe: %u chunks, enqueue %.0f us, total %.0f us\n", n_chunks, t_enq,
+            std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count());
+#endif
     if (mode != MODE_DECRYPT) {
         memcpy(tag_io, c->h_pinned, 16);
         return GCM_OK;
