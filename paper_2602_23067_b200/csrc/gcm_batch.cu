@@ -20,6 +20,10 @@
 // verdicts of both paths come back in one copy.
 #include <cuda_runtime.h>
 #include <string.h>
+#ifdef GCM_PIPE_DEBUG
+#include <chrono>
+#include <stdio.h>
+#endif
 #include <algorithm>
 #include <map>
 #include <mutex>
@@ -482,6 +486,16 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     CUB(guard.err);
     rc = ensure_staging_locked(n);
     if (rc != GCM_OK) return rc;
+#ifdef GCM_PIPE_DEBUG
+    auto T0 = std::chrono::steady_clock::now();
+    auto lap = [&](const char *what) {
+        auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "batch: %-10s %7.1f us\n", what, std::chrono::duration<double, std::micro>(t - T0).count());
+        T0 = t;
+    };
+#else
+    auto lap = [](const char *) {};
+#endif
 
     int first_err = GCM_OK;
     std::vector<uint32_t> small[2], large;                  // small[0]: AES-128, small[1]: AES-256
@@ -516,6 +530,7 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
             pos += count[k];
         }
     }
+    lap("marshal+sort");
     CUB(cudaMemcpyAsync(g.d_desc, g.h_desc, (size_t)n * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
     if (pos) CUB(cudaMemcpyAsync(g.d_order, g.h_order, (size_t)pos * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
     CUB(cudaMemsetAsync(g.d_next, 0, 2 * sizeof(unsigned), s));
@@ -538,7 +553,9 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     // the descriptors hold raw keys: wipe the device copy on the stream, the host copy after the sync
     launch_wipe((uint8_t *)g.d_desc, (uint64_t)n * sizeof(BatchDesc), nullptr, s);
     CUB(cudaGetLastError());
+    lap("enqueue");
     CUB(cudaStreamSynchronize(s));
+    lap("gpu+sync");
     secure_zero(g.h_desc, (size_t)n * sizeof(BatchDesc));
     if (g.by_key.size() > BatchState::kMaxKeys) evict_keys_locked();     // nothing is in flight after the sync
     int failures = 0;
@@ -552,6 +569,7 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
             memcpy(m.tag, g.h_res[i].tag, 16);
         }
     }
+    lap("results");
     if (first_err != GCM_OK) return first_err;
     return decrypt ? failures : GCM_OK;
 }

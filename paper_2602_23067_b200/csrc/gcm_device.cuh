@@ -284,6 +284,10 @@ __device__ __forceinline__ void bulk_copy_g2s(void *dst_smem, const void *src_gm
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Pull a line towards L2 without returning data.  L2 is the coherence point of the device, so a line prefetched
+// before griddepcontrol.wait stays correct even if the previous kernel of the stream still writes it.
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ unsigned long long global_timer_ns()
 {
     unsigned long long t;

@@ -114,6 +114,14 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     const uint32_t r0 = __shfl_sync(0xFFFFFFFFu, (uint32_t)((wg * S) / p.warps), 0);
     const uint32_t r1 = __shfl_sync(0xFFFFFFFFu, (uint32_t)(((wg + 1) * S) / p.warps), 0);
     const bool has_rows = r0 < r1;
+    // HBM latency of the run's first rows is paid now, under the table fill (and, in a train of launches, under
+    // the previous kernel's tail), not after griddepcontrol.wait: prefetch them into L2
+    {
+        const uint32_t f0 = r0 > p.m.fast_lo ? r0 : p.m.fast_lo, f1 = r1 < p.m.fast_hi ? r1 : p.m.fast_hi;
+#pragma unroll
+        for (uint32_t k = 0; k < 2; k++)
+            if (f0 + k < f1) prefetch_l2(p.m.in + 16 * (32ull * (f0 + k) + lane - p.m.base));
+    }
 
     tables_wait(sm);
     STAMP(1);
@@ -162,16 +170,17 @@ gcm_fused_kernel(const __grid_constant__ GcmParams p)
     acc = warp_xor4(gf_mul_mem(acc, wgt));
     // a9: last-CTA-done combination of the CTA partials.  The ticket counter is never reset: the host hands
     // every launch the ticket value that ends it, so an aborted launch cannot leave a stale count behind.
+    // One acquire-release atomic instead of two sequentially consistent fences (__threadfence is MEMBAR.SC + an L1
+    // invalidation, twice on the tail of every launch): the release half publishes this CTA's partial, the acquire
+    // half orders the finisher's reads (L2 reads, __ldcg) behind every other CTA's release.
     unsigned ticket = 0;
     if (lane == 0) {
         p.partials[blockIdx.x] = acc;
-        __threadfence();
-        ticket = atomicAdd(p.counter, 1u);
+        asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(p.counter) : "memory");
     }
     ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
     STAMP(5);
     if (ticket != p.ticket_last) return;
-    __threadfence();
     uint4 tot = make_uint4(0, 0, 0, 0);
     for (uint32_t j = lane; j < gridDim.x; j += 32) tot = xor4(tot, __ldcg(p.partials + j));
     tot = warp_xor4(tot);

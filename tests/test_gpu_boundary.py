@@ -187,3 +187,4 @@ def test_phase_stamps(G):
         assert (live[:, 6] > 0).sum() == 1                    # exactly one CTA finished the message
     finally:
         G.gcm_destroy(ctx)
+
