@@ -3,6 +3,7 @@
     python -m paper_2602_23067_b200.profile_tools summary <report.ncu-rep> <out.txt> "<command that made the report>"
     python -m paper_2602_23067_b200.profile_tools mix     <report.ncu-rep> <out.json> [<key>] "<command>"
     python -m paper_2602_23067_b200.profile_tools static  <kernel name regex> <out.txt>
+    python -m paper_2602_23067_b200.profile_tools launches <ncu launch log.csv> <out.csv> "<command>"
 
 summary  the counters DESIGN.md section 6 quotes, from `ncu -i <report> --page raw --csv`.
 mix      the EXECUTED instruction mix of the row loop per warp-row (32 blocks), from the per-instruction counts of
@@ -111,9 +112,13 @@ def mix(report: str, out: str, key: str, command: str) -> None:
     thread_by_pipe = collections.Counter()
     wf_shared = wf_shared_ideal = 0.0
     total = 0.0
+    issued = 0.0
     for r in rows:
         op = opcode(r["Source"])
-        n = num(r, "Instructions Executed")
+        # predicated-on thread instructions / 32: a warp instruction whose threads are all predicated off (the unused
+        # one of two alternative loads, say) is issued but moves nothing; per block = per thread
+        n = num(r, "Predicated-On Thread Instructions Executed") / 32.0
+        issued += num(r, "Instructions Executed")
         if not op or n == 0:
             continue
         by_op[op] += n
@@ -141,13 +146,14 @@ def mix(report: str, out: str, key: str, command: str) -> None:
         "per_warp_row": {
             "lds32": per_row(lds32), "lds64": per_row(lds64), "lds128": per_row(lds128),
             "ldg128": per_row(ldg128), "stg128": per_row(stg128),
-            "warp_instructions": per_row(total),
+            "warp_instructions": per_row(total), "warp_instructions_issued": per_row(issued),
             "by_pipe_warp_instructions": {k: per_row(v) for k, v in sorted(by_pipe.items())},
             "shared_wavefronts": per_row(wf_shared), "shared_wavefronts_ideal": per_row(wf_shared_ideal),
             "top_opcodes": {k: round(per_row(v), 2) for k, v in by_op.most_common(24)},
         },
         # one warp-row = 32 blocks, one block per lane: warp-level counts per row = thread-level counts per block
-        "note": "whole-kernel executed counts divided by the number of warp-rows (prologue and epilogue included); "
+        "note": "whole-kernel counts (predicated-on thread instructions / 32) divided by the number of warp-rows, prologue and "
+                "epilogue included; warp_instructions_issued counts every issued warp instruction; "
                 "a conflict-free LDS.32 is 1 shared-memory wavefront, an LDS.128 is 4",
     }
     data = {}
@@ -202,11 +208,40 @@ def static(kernel_regex: str, out: str) -> None:
             fo.write("  opcodes: %s\n\n" % ", ".join("%s %d" % kv for kv in ops.most_common(30)))
 
 
+def launches(log: str, out_csv: str, command: str) -> None:
+    """Compact copy of an `ncu --metrics gpu__time_duration.sum --csv` log (kernel names shortened) and the share of
+    device time per kernel, printed as a markdown table."""
+    rows = list(csv.reader(l for l in open(log) if l.startswith('"')))
+    hdr = rows[0]
+    ki, vi, gi, bi = hdr.index("Kernel Name"), hdr.index("Metric Value"), hdr.index("Grid Size"), hdr.index("Block Size")
+    tot, cnt = collections.Counter(), collections.Counter()
+    with open(out_csv, "w") as f:
+        f.write("# %s\n" % command)
+        f.write("id,kernel,grid,block,gpu__time_duration.sum [ns]\n")
+        for r in rows[1:]:
+            try:
+                v = float(r[vi].replace(",", ""))
+            except (ValueError, IndexError):
+                continue
+            name = re.sub(r"^void\s+", "", r[ki])
+            name = re.sub(r"\(.*", "", name)
+            name = re.sub(r"at::<unnamed>::|at::native::|at::", "torch ", name)[:64].strip()
+            f.write("%s,%s,%s,%s,%.0f\n" % (r[0], name.replace(",", ";"), r[gi].replace(",", "x"), r[bi].replace(",", "x"), v))
+            tot[name] += v
+            cnt[name] += 1
+    total = sum(tot.values())
+    print("| kernel | launches | total ns | share |\n|---|---|---|---|")
+    for k, v in tot.most_common():
+        print("| `%s` | %d | %.0f | %.2f %% |" % (k, cnt[k], v, 100 * v / total))
+
+
 def main(argv):
     if len(argv) >= 5 and argv[1] == "summary":
         summary(argv[2], argv[3], argv[4])
     elif len(argv) >= 6 and argv[1] == "mix":
         mix(argv[2], argv[3], argv[4], argv[5])
+    elif len(argv) >= 5 and argv[1] == "launches":
+        launches(argv[2], argv[3], argv[4])
     elif len(argv) >= 4 and argv[1] == "static":
         static(argv[2], argv[3])
     else:
