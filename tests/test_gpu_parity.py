@@ -503,3 +503,36 @@ def test_pipe_rate_probe(G):
     assert 24 <= r["lds32"] <= 33 and 6 <= r["lds128"] <= 8.3
     assert 48 <= r["lop3"] <= 66 and 48 <= r["prmt"] <= 66 and 48 <= r["imad"] <= 66
     assert r["lop3_imad"] > r["lop3"]
+
+
+def test_host_pipeline_chunk_plan_boundaries(G, oracle):
+    """The host pipeline cuts a message into chunks of 2 MiB at both ends, doubling towards the middle; the GHASH
+    state, the chunk powers and the counters have to line up at every cut.  Sizes on and around the cuts (one, two,
+    three ... chunks, a ragged last chunk of 1 byte, of 2 MiB - 1), with and without AAD, encrypt and decrypt."""
+    import os
+    rng = np.random.default_rng(9850)
+    key = rnd(rng, 16).tobytes()
+    MiB = 1 << 20
+    sizes = [2 * MiB - 1, 2 * MiB, 2 * MiB + 1, 4 * MiB, 4 * MiB + 17, 6 * MiB - 1, 6 * MiB + 16, 10 * MiB + 5,
+             14 * MiB, 24 * MiB + 1, 26 * MiB - 16, 40 * MiB + 123457]
+    ctx = G.gcm_init(key)
+    try:
+        for i, n in enumerate(sizes):
+            iv = rnd(rng, 12).tobytes()
+            aad = rnd(rng, [0, 16, 2880, 45][i % 4])
+            pt = workloads.random_payload(rng, n)
+            ref_ct, ref_tag = oracle.gcm_encrypt_threaded(key, iv, aad, pt, threads=os.cpu_count() or 1, segment_blocks=1 << 14)
+            h_pt = torch.from_numpy(pt.copy()).pin_memory()
+            h_ct = torch.empty(n, dtype=torch.uint8).pin_memory()
+            tag = G.gcm_encrypt_host(ctx, iv, aad, h_pt, h_ct)
+            assert tag == ref_tag, n
+            assert np.array_equal(h_ct.numpy(), ref_ct), n
+            back = torch.empty(n, dtype=torch.uint8).pin_memory()
+            assert G.gcm_decrypt_verify_host(ctx, iv, aad, h_ct, back, tag) == G.GCM_OK, n
+            assert torch.equal(back, h_pt), n
+            assert G.gcm_decrypt_verify_host_strict(ctx, iv, aad, h_ct, back, tag) == G.GCM_OK, n
+            h_ct[n - 1] ^= 1
+            assert G.gcm_decrypt_verify_host(ctx, iv, aad, h_ct, back, tag) == G.GCM_ERR_AUTH, n
+            assert not bool(back.any().item())
+    finally:
+        G.gcm_destroy(ctx)
