@@ -14,6 +14,8 @@
 #ifdef GCM_PIPE_DEBUG
 #include <chrono>
 #include <stdio.h>
+#include <stdlib.h>
+static cudaEvent_t dbg_ev[64][4];
 #endif
 
 #include "../../include/gcm.h"
@@ -70,23 +72,26 @@ __global__ void gcm_chunk_pow_kernel(const uint4 *hx, const uint64_t *e, uint32_
     out[k] = gf_to_mem(r);
 }
 
-// Chunk lengths of a message of `len` bytes.  The first upload and the last download cannot overlap with anything,
-// so the plan starts and ends with PIPE_MIN_CHUNK_BYTES; chunks double up to the middle size (about len / 12, at
-// most PIPE_CHUNK_BYTES) and come down again by a factor of about 0.6, slowly enough that a chunk's download is
-// over before the upload two chunks later wants its slot (s_k <= s_(k+1) + s_(k+2)).  Every chunk but the last is
-// a multiple of PIPE_MIN_CHUNK_BYTES (so of 16); the last one takes the ragged end.
+// Chunk lengths of a message of `len` bytes.  Measured on the B200 box (per-chunk event timeline, 64 MiB message):
+// with both directions busy every copy costs about 30 us on top of its bytes at 50 GB/s (a 4 MiB copy takes 113 us,
+// not 84), so the plan wants FEW chunks, while the first upload and the last download, which overlap with nothing,
+// want SMALL ones.  Hence: PIPE_MIN_CHUNK_BYTES at both ends, doubling up to the middle size (about len / 4, at most
+// PIPE_CHUNK_BYTES) and coming down again by a factor of about 0.6, slowly enough that a chunk's download is over
+// before the upload two chunks later wants its slot (s_k <= s_(k+1) + s_(k+2)).  Every chunk but the last is a
+// multiple of PIPE_MIN_CHUNK_BYTES (so of 16); the last one takes the ragged end.
 static uint32_t plan_chunks(uint64_t len, uint64_t *plan)
 {
     if (len == 0) { plan[0] = 0; return 1; }
     const uint64_t U = PIPE_MIN_CHUNK_BYTES;
     uint64_t mid = U;
-    while (mid * 2 <= len / 12 && mid * 2 <= PIPE_CHUNK_BYTES) mid *= 2;
+    while (mid * 2 <= len / 4 && mid * 2 <= PIPE_CHUNK_BYTES) mid *= 2;
     uint64_t back[PIPE_MAX_CHUNKS];
     uint32_t nf = 0, nb = 0;
     const uint64_t last = ((len - 1) % U) + 1;
     uint64_t rem = len - last;
     back[nb++] = last;
-    uint64_t a = U, b = U;
+    uint64_t a = U, b = (U * 8 / 5 + U - 1) / U * U;
+    if (b > mid) b = mid;
     while (rem > 0) {
         uint64_t t = a < rem ? a : rem;
         plan[nf++] = t; rem -= t;
@@ -211,7 +216,13 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         cudaStream_t s = hp->stream[slot];
         const uint64_t clen = plan[k];
         const bool first = (k == 0), last = (k == n_chunks - 1);
+#ifdef GCM_PIPE_DEBUG
+        if (k < 64) { for (int q = 0; q < 4; q++) if (!dbg_ev[k][q]) cudaEventCreate(&dbg_ev[k][q]); cudaEventRecord(dbg_ev[k][0], s); }
+#endif
         if (clen) CU(cudaMemcpyAsync(hp->d_stage[slot], (const uint8_t *)h_in + off, clen, cudaMemcpyHostToDevice, s));
+#ifdef GCM_PIPE_DEBUG
+        if (k < 64) cudaEventRecord(dbg_ev[k][1], s);
+#endif
         // kernels run in message order: chunk k needs chunk k-1's GHASH state (and the powers)
         if (!first) CU(cudaStreamWaitEvent(s, hp->kernel_done[(k - 1) % PIPE_SLOTS], 0));
         else if (n_chunks > 1) CU(cudaStreamWaitEvent(s, hp->kernel_done[PIPE_SLOTS - 1], 0));
@@ -235,8 +246,14 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         memset(&p, 0, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
         CU(cudaEventRecord(hp->kernel_done[slot], s));
+#ifdef GCM_PIPE_DEBUG
+        if (k < 64) cudaEventRecord(dbg_ev[k][2], s);
+#endif
         if (d_sum32 && mode == MODE_ENCRYPT) CU(launch_fits_sum32(hp->d_stage[slot], clen, d_sum32, c->sm_count, s));
         if (clen && mode != MODE_GHASH) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
+#ifdef GCM_PIPE_DEBUG
+        if (k < 64) cudaEventRecord(dbg_ev[k][3], s);
+#endif
     }
 #ifdef GCM_PIPE_DEBUG
     const double t_enq = std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count();
@@ -245,6 +262,13 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
 #ifdef GCM_PIPE_DEBUG
     fprintf(stderr, "pipe: %u chunks, enqueue %.0f us, total %.0f us\n", n_chunks, t_enq,
             std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count());
+    if (getenv("GCM_PIPE_TIMELINE"))
+        for (uint32_t k = 0; k < n_chunks && k < 64; k++) {
+            float a, b, c2, d2;
+            cudaEventElapsedTime(&a, dbg_ev[0][0], dbg_ev[k][0]); cudaEventElapsedTime(&b, dbg_ev[0][0], dbg_ev[k][1]);
+            cudaEventElapsedTime(&c2, dbg_ev[0][0], dbg_ev[k][2]); cudaEventElapsedTime(&d2, dbg_ev[0][0], dbg_ev[k][3]);
+            fprintf(stderr, "  chunk %2u %6.2f MiB: h2d start %7.1f end %7.1f | kernel end %7.1f | d2h end %7.1f us\n", k, plan[k] / 1048576.0, a * 1e3, b * 1e3, c2 * 1e3, d2 * 1e3);
+        }
 #endif
     if (mode != MODE_DECRYPT) {
         memcpy(tag_io, c->h_pinned, 16);
