@@ -618,6 +618,14 @@ def run_extra(args):
             rc = G.gcm._L.gcm_encrypt_batch(arr, cnt, sp)
             assert rc == 0
         total_ms, per, clocks = timed(step)
+        # the same batch through the device-descriptor call: descriptors packed and uploaded once, asynchronous launches,
+        # nothing marshalled per call (ordering kernel + warp-per-message kernel inside the event pair)
+        d_msgs = torch.from_numpy(G.gcm_pack_dmsgs(batch).view(np.uint8).copy()).cuda()
+        dev_ms, _, _ = timed(lambda: G.gcm_encrypt_batch_device(d_msgs, len(batch), stream))
+        host_tags = bytes(arr[0].tag)
+        assert d_msgs.cpu().numpy().view(G.gcm_dmsg_dtype())["tag"][0].tobytes() == host_tags
+        line["device_descriptors"] = {"value": steps * nbytes / (dev_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": dev_ms / steps,
+                                      "how": "gcm_encrypt_batch_device: gcm_dmsg array resident on the device, asynchronous, device-timed"}
         G.gcm_batch_release()
         gbs = steps * nbytes / (total_ms * 1e-3) / 1e9
         pb = pipe_bound_gbs("batch_aes128_enc", 10, sm_count, sm_mhz, G.gcm_measure_pipe_rates())

@@ -243,6 +243,38 @@ typedef struct {
 GCM_API int gcm_encrypt_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
 GCM_API int gcm_decrypt_verify_batch(gcm_msg *msgs, uint32_t n, void *cuda_stream);
 
+/*
+ * Device-descriptor form of the batched calls, for many short messages (config C4): the descriptors
+ * themselves live in DEVICE memory, so a call marshals nothing on the host (for 10,000 messages that is a quarter of
+ * the synchronous call's time) and does not synchronise: one small kernel orders the messages longest first, one
+ * persistent warp-per-message kernel per key size does the work, and every message's tag (encrypt) and verdict are
+ * written into its own descriptor.  The caller fills the array once (keys included: it is the caller's to wipe) and
+ * may launch it any number of times.
+ *   key       16 or 32 bytes used          key_bits  128 or 256 (anything else: status = GCM_ERR_ARG, message skipped)
+ *   tag       out (encrypt) / in (decrypt) status    out: GCM_OK / GCM_ERR_AUTH (output zero-filled) / GCM_ERR_ARG
+ *   iv        12 bytes                     d_aad / d_in / d_out (device), aad_len, len as in gcm_msg
+ * Every message is handled by one warp whatever its length: meant for messages up to a few hundred KiB (longer ones
+ * are correct but slow; use gcm_encrypt_batch for FITS-sized messages).  Length limits and overlap rules are the
+ * caller's to keep (the descriptors cannot be checked from the host).  Calls on different streams are ordered behind
+ * each other by the library.  Returns GCM_OK or a negative error for the launch itself.
+ */
+typedef struct {
+    uint8_t     key[32];
+    uint8_t     tag[16];
+    int32_t     status;
+    uint32_t    key_bits;
+    uint8_t     iv[12];
+    uint32_t    reserved;
+    const void *d_aad;
+    const void *d_in;
+    void       *d_out;
+    uint64_t    aad_len;
+    uint64_t    len;
+} gcm_dmsg;                     /* 112 bytes */
+
+GCM_API int gcm_encrypt_batch_device(gcm_dmsg *d_msgs, uint32_t n, void *cuda_stream);
+GCM_API int gcm_decrypt_verify_batch_device(gcm_dmsg *d_msgs, uint32_t n, void *cuda_stream);
+
 /* Frees the batch path's cached per-key contexts and staging buffers (zeroising key material) and the
  * wiped allocations that gcm_destroy keeps for the next gcm_init. */
 GCM_API void gcm_batch_release(void);

@@ -20,6 +20,7 @@
 // verdicts of both paths come back in one copy.
 #include <cuda_runtime.h>
 #include <string.h>
+#include <stddef.h>
 #ifdef GCM_PIPE_DEBUG
 #include <chrono>
 #include <stdio.h>
@@ -48,24 +49,34 @@
 #define BATCH_SMEM_BYTES   (BATCH_HP_OFF + BATCH_WARPS * BATCH_HP_BYTES)
 #define BATCH_LARGE_BYTES  (256ull << 10)                /* at and above: fused kernel per message */
 
-struct BatchDesc {            // one per message, device; 112 bytes so that tag stays 16-byte aligned
+struct BatchDesc {            // one per message, device; == gcm_dmsg of include/gcm.h (the device-descriptor calls hand it over as is)
     uint32_t key[8];
-    uint32_t tag[4];          // decrypt: expected tag
+    uint32_t tag[4];          // decrypt: expected tag; device-descriptor encrypt: the tag goes here
+    int32_t  status;          // device-descriptor calls: the verdict goes here
+    uint32_t key_bits;        // device-descriptor calls: 128 / 256 (the host path sorts by key size itself)
     uint32_t iv[3];
-    uint32_t pad32;
+    uint32_t reserved;
     const uint8_t *aad;
     const uint8_t *in;
     uint8_t *out;
     uint64_t aad_len;
     uint64_t len;
-    uint64_t pad64;
 };
-static_assert(sizeof(BatchDesc) == 112, "BatchDesc layout");
-struct BatchResult {          // one per message, device
+static_assert(sizeof(BatchDesc) == 112 && sizeof(gcm_dmsg) == 112, "BatchDesc / gcm_dmsg layout");
+static_assert(offsetof(BatchDesc, tag) == offsetof(gcm_dmsg, tag) && offsetof(BatchDesc, status) == offsetof(gcm_dmsg, status) &&
+              offsetof(BatchDesc, key_bits) == offsetof(gcm_dmsg, key_bits) && offsetof(BatchDesc, iv) == offsetof(gcm_dmsg, iv) &&
+              offsetof(BatchDesc, aad) == offsetof(gcm_dmsg, d_aad) && offsetof(BatchDesc, out) == offsetof(gcm_dmsg, d_out) &&
+              offsetof(BatchDesc, len) == offsetof(gcm_dmsg, len), "BatchDesc / gcm_dmsg layout");
+struct BatchOut {             // where a message's result goes: tag, then verdict
+    uint32_t tag[4];
+    int status;
+};
+struct BatchResult {          // one per message, device (host-descriptor path): a BatchOut padded to 32 bytes
     uint32_t tag[4];
     int status;
     int pad[3];
 };
+static_assert(offsetof(BatchDesc, status) == offsetof(BatchDesc, tag) + 16, "a BatchOut sits inside a BatchDesc");
 static_assert(sizeof(BatchResult) == sizeof(MultiResult), "BatchResult / MultiResult layout");
 
 // ---- device ---------------------------------------------------------------------------------------
@@ -111,7 +122,7 @@ __device__ __forceinline__ uint4 shfl4(uint4 v, uint32_t src)
 }
 
 template <int NR, int MODE>
-__device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *res, const uint8_t *sm,
+__device__ __forceinline__ void batch_message(const BatchDesc &d, BatchOut *res, const uint8_t *sm,
                                               uint8_t *tab, uint4 *hp, uint32_t lane)
 {
     const uint32_t lane4 = lane * 4;
@@ -198,14 +209,19 @@ __device__ __forceinline__ void batch_message(const BatchDesc &d, BatchResult *r
 // order[j]: message index of the j-th ticket (longest first); next: ticket counter.
 struct Te0Param { uint32_t w[256]; };      // the round table T0 by value: constant bank, no global load at kernel start
 
+// results: message m's BatchOut is at res_base + m * res_stride (the separate result array of the host-descriptor
+// path, or the tag / status fields of the descriptor itself).  n_dev (may be NULL): the ticket count lives on the
+// device (written by gcm_batch_order_kernel).
 template <int NR, int MODE>
 __global__ void __launch_bounds__(BATCH_THREADS, 1)
-gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *order, uint32_t n,
-                 unsigned *next, const __grid_constant__ Te0Param te0)
+gcm_batch_kernel(const BatchDesc *descs, uint8_t *res_base, uint32_t res_stride, const uint32_t *order, uint32_t n,
+                 const unsigned *n_dev, unsigned *next, const __grid_constant__ Te0Param te0)
 {
     extern __shared__ __align__(1024) uint8_t sm[];
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t warp = __shfl_sync(0xFFFFFFFFu, threadIdx.x >> 5, 0);
+    if (n_dev != nullptr) n = *n_dev;
+    if (n == 0) return;
     fill_aes_tables<BATCH_THREADS>(sm, te0.w, threadIdx.x);
     __syncthreads();
     uint8_t *tab = sm + BATCH_TAB_OFF + warp * BATCH_TAB_BYTES;
@@ -217,21 +233,64 @@ gcm_batch_kernel(const BatchDesc *descs, BatchResult *results, const uint32_t *o
         if (j >= n) break;
         const uint32_t m = __ldg(order + j);
         BatchDesc d = descs[m];
-        batch_message<NR, MODE>(d, results + m, sm, tab, hp, lane);
+        batch_message<NR, MODE>(d, reinterpret_cast<BatchOut *>(res_base + (size_t)m * res_stride), sm, tab, hp, lane);
         __syncwarp();
     }
 }
 
 template <int NR, int MODE>
-static cudaError_t launch_batch(int blocks, const BatchDesc *descs, BatchResult *results, const uint32_t *order,
-                                uint32_t n, unsigned *next, const Te0Param &te0, cudaStream_t s)
+static cudaError_t launch_batch(int blocks, const BatchDesc *descs, uint8_t *res_base, uint32_t res_stride, const uint32_t *order,
+                                uint32_t n, const unsigned *n_dev, unsigned *next, const Te0Param &te0, cudaStream_t s)
 {
     static std::atomic<bool> configured[GCM_MAX_DEVICES];
     auto kern = gcm_batch_kernel<NR, MODE>;
     cudaError_t e = ensure_smem_attr((const void *)kern, configured, BATCH_SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    kern<<<blocks, BATCH_THREADS, BATCH_SMEM_BYTES, s>>>(descs, results, order, n, next, te0);
+    kern<<<blocks, BATCH_THREADS, BATCH_SMEM_BYTES, s>>>(descs, res_base, res_stride, order, n, n_dev, next, te0);
     return cudaGetLastError();
+}
+
+// Device-descriptor calls: ticket order (longest first, by 512-byte rows) for the two key sizes, made on the device.
+// One CTA: histogram over (key size, row count), exclusive scan, scatter.  order[0 .. n) holds the AES-128 messages,
+// order[n .. 2n) the AES-256 ones; counts[0 / 1] how many of each; descriptors with any other key_bits get
+// status GCM_ERR_ARG and are left out.  ctr[0..3] = ticket counters and counts, zeroed / written here.
+#define ORDER_BUCKETS 514
+__global__ void __launch_bounds__(1024, 1)
+gcm_batch_order_kernel(BatchDesc *descs, uint32_t n, uint32_t *order, unsigned *ctr)
+{
+    __shared__ unsigned hist[2][ORDER_BUCKETS];
+    __shared__ unsigned total[2];
+    const uint32_t t = threadIdx.x;
+    for (uint32_t i = t; i < 2 * ORDER_BUCKETS; i += blockDim.x) (&hist[0][0])[i] = 0;
+    __syncthreads();
+    auto bucket = [](uint64_t len) {          // descending: the longest messages get the lowest bucket
+        const uint64_t rows = (len + 511) / 512;
+        return (uint32_t)(ORDER_BUCKETS - 1 - (rows < ORDER_BUCKETS - 1 ? rows : ORDER_BUCKETS - 1));
+    };
+    for (uint32_t i = t; i < n; i += blockDim.x) {
+        const uint32_t kb = descs[i].key_bits;
+        if (kb == 128 || kb == 256) {
+            atomicAdd(&hist[kb == 256][bucket(descs[i].len)], 1u);
+            descs[i].status = GCM_STATUS_PENDING;          // reads "refused" until the message's warp has written it
+        } else {
+            descs[i].status = GCM_ERR_ARG;
+        }
+    }
+    __syncthreads();
+    if (t < 2) {                               // exclusive scan per key size (514 entries: not worth a parallel scan)
+        unsigned run = 0;
+        for (int b = 0; b < ORDER_BUCKETS; b++) { const unsigned c = hist[t][b]; hist[t][b] = run; run += c; }
+        total[t] = run;
+    }
+    __syncthreads();
+    for (uint32_t i = t; i < n; i += blockDim.x) {
+        const uint32_t kb = descs[i].key_bits;
+        if (kb != 128 && kb != 256) continue;
+        const unsigned cls = kb == 256;
+        const unsigned pos = atomicAdd(&hist[cls][bucket(descs[i].len)], 1u);
+        order[(size_t)cls * n + pos] = i;
+    }
+    if (t == 0) { ctr[0] = 0; ctr[1] = 0; ctr[2] = total[0]; ctr[3] = total[1]; }
 }
 
 // ---- host -----------------------------------------------------------------------------------------
@@ -249,7 +308,9 @@ struct BatchState {
     BatchDesc *h_desc = nullptr, *d_desc = nullptr;
     BatchResult *h_res = nullptr, *d_res = nullptr;
     uint32_t *h_order = nullptr, *d_order = nullptr;
-    unsigned *d_next = nullptr;      // [2]
+    unsigned *d_next = nullptr;      // [4]: two ticket counters; the device-descriptor calls add the two ticket counts
+    cudaEvent_t dev_done = nullptr;  // last device-descriptor call: its kernels still read the order lists and counters
+    bool dev_pending = false;
     uint32_t *d_te0 = nullptr;
     Te0Param h_te0;                  // host copy of the round table (made on the device by gcm_te0_kernel)
     // staging of the large-message path (gcm_multi.cu): descriptors, chunks, per-warp chunk ranges,
@@ -278,6 +339,7 @@ void free_staging_locked()
     if (g.d_order) cudaFree(g.d_order);
     if (g.h_order) cudaFreeHost(g.h_order);
     if (g.d_next) cudaFree(g.d_next);
+    if (g.dev_done) { cudaEventSynchronize(g.dev_done); cudaEventDestroy(g.dev_done); g.dev_done = nullptr; g.dev_pending = false; }
     if (g.d_te0) cudaFree(g.d_te0);
     if (g.d_multi) cudaFree(g.d_multi);
     if (g.h_multi) cudaFreeHost(g.h_multi);
@@ -317,8 +379,9 @@ int ensure_staging_locked(uint32_t n)
             if ((e = cudaHostAlloc((void **)&g.h_res, (size_t)cap * sizeof(BatchResult), cudaHostAllocDefault)) != cudaSuccess) break;
             if ((e = cudaMalloc((void **)&g.d_res, (size_t)cap * sizeof(BatchResult))) != cudaSuccess) break;
             if ((e = cudaHostAlloc((void **)&g.h_order, (size_t)cap * sizeof(uint32_t), cudaHostAllocDefault)) != cudaSuccess) break;
-            if ((e = cudaMalloc((void **)&g.d_order, (size_t)cap * sizeof(uint32_t))) != cudaSuccess) break;
-            if ((e = cudaMalloc((void **)&g.d_next, 2 * sizeof(unsigned))) != cudaSuccess) break;
+            if ((e = cudaMalloc((void **)&g.d_order, 2 * (size_t)cap * sizeof(uint32_t))) != cudaSuccess) break;   // x 2: the device-descriptor calls keep one list per key size
+            if ((e = cudaMalloc((void **)&g.d_next, 4 * sizeof(unsigned))) != cudaSuccess) break;
+            if (!g.dev_done && (e = cudaEventCreateWithFlags(&g.dev_done, cudaEventDisableTiming)) != cudaSuccess) break;
             if ((e = cudaMalloc((void **)&g.d_te0, 256 * sizeof(uint32_t))) != cudaSuccess) break;
             launch_te0(g.d_te0, 0);
             if ((e = cudaGetLastError()) != cudaSuccess) break;
@@ -486,6 +549,7 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     CUB(guard.err);
     rc = ensure_staging_locked(n);
     if (rc != GCM_OK) return rc;
+    if (g.dev_pending) { CUB(cudaStreamWaitEvent(s, g.dev_done, 0)); g.dev_pending = false; }
 #ifdef GCM_PIPE_DEBUG
     auto T0 = std::chrono::steady_clock::now();
     auto lap = [&](const char *what) {
@@ -541,10 +605,10 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
         const uint32_t want = (count[k] + BATCH_WARPS - 1) / BATCH_WARPS;
         const int blocks = (int)std::min<uint32_t>(want, (uint32_t)g.sm_count);
         cudaError_t e;
-        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s)
-                                : launch_batch<10, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s);
-        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s)
-                                : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, g.d_res, g.d_order + start[k], count[k], g.d_next + k, g.h_te0, s);
+        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, g.d_desc, (uint8_t *)g.d_res, (uint32_t)sizeof(BatchResult), g.d_order + start[k], count[k], nullptr, g.d_next + k, g.h_te0, s)
+                                : launch_batch<10, MODE_ENCRYPT>(blocks, g.d_desc, (uint8_t *)g.d_res, (uint32_t)sizeof(BatchResult), g.d_order + start[k], count[k], nullptr, g.d_next + k, g.h_te0, s);
+        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, g.d_desc, (uint8_t *)g.d_res, (uint32_t)sizeof(BatchResult), g.d_order + start[k], count[k], nullptr, g.d_next + k, g.h_te0, s)
+                                : launch_batch<14, MODE_ENCRYPT>(blocks, g.d_desc, (uint8_t *)g.d_res, (uint32_t)sizeof(BatchResult), g.d_order + start[k], count[k], nullptr, g.d_next + k, g.h_te0, s);
         if (e != cudaSuccess) return gcm_cuda_fail(e);
     }
     rc = run_large_locked(msgs, large, decrypt, s, &first_err);
@@ -575,6 +639,46 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
 }
 
 }  // namespace
+
+// Device-descriptor calls (include/gcm.h: gcm_dmsg): nothing is marshalled on the host.  One small kernel orders the
+// tickets, then one persistent warp-per-message kernel per key size; tags and verdicts land in the descriptors.
+static int run_batch_device(gcm_dmsg *d_msgs, uint32_t n, void *stream, bool decrypt)
+{
+    if (n && !d_msgs) return GCM_ERR_ARG;
+    if (n == 0) return GCM_OK;
+    std::lock_guard<std::mutex> lock(g.mu);
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0;
+    int rc = gcm_default_device(&dev);
+    if (rc != GCM_OK) return rc;
+    DeviceGuard guard(dev);
+    CUB(guard.err);
+    rc = ensure_staging_locked(n);
+    if (rc != GCM_OK) return rc;
+    // the previous device-descriptor call may still be reading the order lists and counters
+    if (g.dev_pending) CUB(cudaStreamWaitEvent(s, g.dev_done, 0));
+    BatchDesc *descs = reinterpret_cast<BatchDesc *>(d_msgs);
+    gcm_batch_order_kernel<<<1, 1024, 0, s>>>(descs, n, g.d_order, g.d_next);
+    CUB(cudaGetLastError());
+    uint8_t *res_base = reinterpret_cast<uint8_t *>(d_msgs) + offsetof(BatchDesc, tag);
+    const uint32_t want = (n + BATCH_WARPS - 1) / BATCH_WARPS;
+    const int blocks = (int)std::min<uint32_t>(want, (uint32_t)g.sm_count);
+    for (int k = 0; k < 2; k++) {
+        cudaError_t e;
+        const uint32_t *order = g.d_order + (size_t)k * n;
+        if (k == 0) e = decrypt ? launch_batch<10, MODE_DECRYPT>(blocks, descs, res_base, (uint32_t)sizeof(BatchDesc), order, n, g.d_next + 2, g.d_next, g.h_te0, s)
+                                : launch_batch<10, MODE_ENCRYPT>(blocks, descs, res_base, (uint32_t)sizeof(BatchDesc), order, n, g.d_next + 2, g.d_next, g.h_te0, s);
+        else        e = decrypt ? launch_batch<14, MODE_DECRYPT>(blocks, descs, res_base, (uint32_t)sizeof(BatchDesc), order, n, g.d_next + 3, g.d_next + 1, g.h_te0, s)
+                                : launch_batch<14, MODE_ENCRYPT>(blocks, descs, res_base, (uint32_t)sizeof(BatchDesc), order, n, g.d_next + 3, g.d_next + 1, g.h_te0, s);
+        if (e != cudaSuccess) return gcm_cuda_fail(e);
+    }
+    CUB(cudaEventRecord(g.dev_done, s));
+    g.dev_pending = true;
+    return GCM_OK;
+}
+
+extern "C" int gcm_encrypt_batch_device(gcm_dmsg *d_msgs, uint32_t n, void *stream) { return run_batch_device(d_msgs, n, stream, false); }
+extern "C" int gcm_decrypt_verify_batch_device(gcm_dmsg *d_msgs, uint32_t n, void *stream) { return run_batch_device(d_msgs, n, stream, true); }
 
 extern "C" void gcm_batch_release(void)
 {

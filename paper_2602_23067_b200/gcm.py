@@ -23,6 +23,7 @@ EXPORTED_SYMBOLS = [
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
     "gcm_encrypt_host", "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
+    "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device",
     "gcm_measure_pipe_rates",
 ]
 RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad"]
@@ -87,6 +88,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_set_phase_stamps.argtypes = [vp, vp]
     L.gcm_encrypt_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
+    L.gcm_encrypt_batch_device.argtypes = [vp, ctypes.c_uint32, vp]
+    L.gcm_decrypt_verify_batch_device.argtypes = [vp, ctypes.c_uint32, vp]
     L.gcm_batch_release.argtypes = []
     L.gcm_batch_release.restype = None
     L.gcm_measure_pipe_rates.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
@@ -363,6 +366,63 @@ def gcm_decrypt_verify_batch(msgs: Iterable[dict], stream=None) -> List[int]:
         raise GcmError(rc, "gcm_decrypt_verify_batch")
     del keep
     return [arr[i].status for i in range(n)]
+
+
+GCM_DMSG_BYTES = 112
+
+
+def gcm_dmsg_dtype():
+    """numpy structured dtype of struct gcm_dmsg (include/gcm.h), 112 bytes."""
+    import numpy as np
+    return np.dtype([("key", np.uint8, 32), ("tag", np.uint8, 16), ("status", np.int32), ("key_bits", np.uint32),
+                     ("iv", np.uint8, 12), ("reserved", np.uint32), ("d_aad", np.uint64), ("d_in", np.uint64),
+                     ("d_out", np.uint64), ("aad_len", np.uint64), ("len", np.uint64)])
+
+
+def gcm_pack_dmsgs(msgs: Iterable[dict]):
+    """Host array of gcm_dmsg records from dicts with key, iv, aad (device or None), input, output (device) and, for
+    decryption, tag.  Marshalling only; copy it to the device (torch.from_numpy(a.view(numpy.uint8)).cuda()) and hand
+    that tensor to gcm_encrypt_batch_device / gcm_decrypt_verify_batch_device."""
+    import numpy as np
+    msgs = list(msgs)
+    a = np.zeros(len(msgs), dtype=gcm_dmsg_dtype())
+    assert a.dtype.itemsize == GCM_DMSG_BYTES
+    for i, m in enumerate(msgs):
+        key = bytes(m["key"])
+        a["key"][i, :len(key)] = np.frombuffer(key, np.uint8)[:32]
+        a["key_bits"][i] = 8 * len(key)
+        a["iv"][i] = np.frombuffer(_iv(m["iv"]), np.uint8)
+        a_ptr, a_len = _dev(m.get("aad"))
+        i_ptr, i_len = _dev(m["input"])
+        o_ptr, o_len = _dev(m["output"])
+        if o_len != i_len:
+            raise ValueError("message %d: input and output sizes differ" % i)
+        a["d_aad"][i], a["aad_len"][i] = a_ptr or 0, a_len
+        a["d_in"][i], a["len"][i] = i_ptr or 0, i_len
+        a["d_out"][i] = o_ptr or 0
+        if "tag" in m and m["tag"] is not None:
+            a["tag"][i] = np.frombuffer(_tag(m["tag"]), np.uint8)
+    return a
+
+
+def _dmsgs(d_msgs, n):
+    ptr, nbytes = _dev(d_msgs)
+    if n is None:
+        n = nbytes // GCM_DMSG_BYTES
+    if nbytes < n * GCM_DMSG_BYTES:
+        raise ValueError("d_msgs holds fewer than n descriptors")
+    return ptr, int(n)
+
+
+def gcm_encrypt_batch_device(d_msgs, n: Optional[int] = None, stream=None) -> None:
+    """Asynchronous; tags and statuses land in the device-resident descriptors (gcm_dmsg)."""
+    ptr, n = _dmsgs(d_msgs, n)
+    _check(_L.gcm_encrypt_batch_device(ptr, n, _stream(stream)), "gcm_encrypt_batch_device")
+
+
+def gcm_decrypt_verify_batch_device(d_msgs, n: Optional[int] = None, stream=None) -> None:
+    ptr, n = _dmsgs(d_msgs, n)
+    _check(_L.gcm_decrypt_verify_batch_device(ptr, n, _stream(stream)), "gcm_decrypt_verify_batch_device")
 
 
 def gcm_batch_release() -> None:

@@ -151,6 +151,17 @@ def test_config_c4_full_batch(G, oracle):
         assert np.array_equal(out[o: o + m.payload.size], ref_ct), m.name
         pad_end = (m.payload.size + 15) // 16 * 16
         assert not out[o + m.payload.size: o + pad_end].any(), "%s: wrote past len" % m.name
+    # the same 10,000 messages through the device-descriptor call (ordering on the device, tags in the descriptors)
+    d_out2 = torch.zeros_like(d_in)
+    host = G.gcm_pack_dmsgs([dict(b, output=d_out2[o: o + m.payload.size]) for b, m, o in zip(batch, msgs, offs)])
+    d_msgs = torch.from_numpy(host.view(np.uint8).copy()).cuda()
+    G.gcm_encrypt_batch_device(d_msgs)
+    torch.cuda.synchronize()
+    res = d_msgs.cpu().numpy().view(host.dtype)
+    assert torch.equal(d_out2, d_out), "device-descriptor ciphertext differs from the host-descriptor call's"
+    assert not res["status"].any()
+    for m, (_, ref_tag), i in zip(msgs, refs, range(len(msgs))):
+        assert res["tag"][i].tobytes() == ref_tag, m.name
     # decrypt + verify the whole batch, three seeded forgeries (ciphertext, tag, AAD)
     d_back = torch.zeros_like(d_in)
     dec = [{"key": b["key"], "iv": b["iv"], "aad": b["aad"], "input": b["output"],

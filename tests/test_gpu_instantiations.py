@@ -190,3 +190,81 @@ def test_ghash_only_long_ragged(G, oracle, geometry):
         assert d_s.cpu().numpy().tobytes() == oracle.ghash_segmented(h, aad, c, 1 << 16, THREADS)
     finally:
         G.gcm_destroy(ctx)
+
+
+def test_batch_device_descriptors(G, oracle):
+    """gcm_encrypt_batch_device / gcm_decrypt_verify_batch_device: descriptors resident on the device, ordering done
+    by a kernel, tags and verdicts written into the descriptors.  Both key sizes in one call, every tail shape,
+    empty messages, empty AAD, unaligned buffers, a descriptor with a bad key size, the same array launched twice,
+    then decryption with three forgeries: refused, zero-filled, neighbours untouched.  Byte-exact against the oracle."""
+    import workloads
+    rng = np.random.default_rng(9940)
+    lens = [0, 1, 15, 16, 17, 31, 32, 33, 495, 496, 497, 511, 512, 513, 4096, 8191, 8192 + 5, 16 * 32 * 7 + 16 * 30 + 9,
+            65536, 70001, 200000, 300000] + rng.integers(1, 65537, 60).tolist()
+    specs = []
+    for i, n in enumerate(lens):
+        klen = 16 if i % 3 else 32
+        a = [0, 1, 16, 17, 100, 256, 2880][i % 7]
+        specs.append((rnd(rng, klen).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, a), rnd(rng, n), i % 5 == 4))
+    offs, pos = [], 0
+    for (_, _, _, pt, unal) in specs:
+        pos = (pos + 15) // 16 * 16 + (3 if unal else 0)
+        offs.append(pos)
+        pos += len(pt) + 16
+    big_in = torch.zeros(pos + 16, dtype=torch.uint8, device="cuda")
+    big_out = torch.zeros(pos + 16, dtype=torch.uint8, device="cuda")
+    for (_, _, _, pt, _), o in zip(specs, offs):
+        if len(pt):
+            big_in[o: o + len(pt)] = dev(pt)
+    aads = [dev(aad) if len(aad) else None for (_, _, aad, _, _) in specs]
+    msgs = [{"key": key, "iv": iv, "aad": d_aad, "input": big_in[o: o + len(pt)], "output": big_out[o: o + len(pt)]}
+            for (key, iv, aad, pt, _), o, d_aad in zip(specs, offs, aads)]
+    host = G.gcm_pack_dmsgs(msgs)
+    assert host.dtype.itemsize == G.GCM_DMSG_BYTES == 112
+    bad = len(msgs) // 2
+    host["key_bits"][bad] = 192                                   # not a key size of reading S1
+    d_msgs = torch.from_numpy(host.view(np.uint8).copy()).cuda()
+    for _ in range(2):                                            # the same descriptor array twice
+        G.gcm_encrypt_batch_device(d_msgs)
+    torch.cuda.synchronize()
+    res = d_msgs.cpu().numpy().view(host.dtype)
+    out = big_out.cpu().numpy()
+    covered = np.zeros(out.size, bool)
+    refs = []
+    for i, ((key, iv, aad, pt, _), o) in enumerate(zip(specs, offs)):
+        ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
+        refs.append((ref_ct, ref_tag))
+        if i == bad:
+            assert int(res["status"][i]) == G.GCM_ERR_ARG
+            assert not out[o: o + len(pt)].any(), "a refused descriptor was processed"
+            continue
+        assert int(res["status"][i]) == G.GCM_OK, i
+        assert res["tag"][i].tobytes() == ref_tag, "tag len=%d aad=%d" % (len(pt), len(aad))
+        assert np.array_equal(out[o: o + len(pt)], ref_ct), "ct len=%d aad=%d" % (len(pt), len(aad))
+        covered[o: o + len(pt)] = True
+    assert not out[~covered].any(), "wrote outside a message's output range"
+    # decrypt through device descriptors: oracle ciphertext in, three forgeries
+    ct_in = torch.zeros_like(big_in)
+    for (ref_ct, _), o in zip(refs, offs):
+        if ref_ct.size:
+            ct_in[o: o + ref_ct.size] = dev(ref_ct)
+    dec_out = torch.full_like(big_out, 0x77)
+    dmsgs = [{"key": key, "iv": iv, "aad": d_aad, "input": ct_in[o: o + len(pt)], "output": dec_out[o: o + len(pt)], "tag": ref_tag}
+             for (key, iv, aad, pt, _), o, d_aad, (_, ref_tag) in zip(specs, offs, aads, refs)]
+    forged = {5, 9, 20}
+    t = bytearray(dmsgs[5]["tag"]); t[15] ^= 1; dmsgs[5]["tag"] = bytes(t)
+    ct_in[offs[9] + len(specs[9][3]) // 2] ^= 0x10
+    a20 = dmsgs[20]["aad"].clone(); a20[0] ^= 0x80; dmsgs[20]["aad"] = a20
+    d_dec = torch.from_numpy(G.gcm_pack_dmsgs(dmsgs).view(np.uint8).copy()).cuda()
+    G.gcm_decrypt_verify_batch_device(d_dec)
+    torch.cuda.synchronize()
+    st = d_dec.cpu().numpy().view(host.dtype)["status"]
+    got = dec_out.cpu().numpy()
+    for i, ((key, iv, aad, pt, _), o) in enumerate(zip(specs, offs)):
+        if i in forged:
+            assert int(st[i]) == G.GCM_ERR_AUTH, i
+            assert not got[o: o + len(pt)].any(), "message %d not suppressed" % i
+        else:
+            assert int(st[i]) == G.GCM_OK, i
+            assert np.array_equal(got[o: o + len(pt)], pt), i
+    G.gcm_batch_release()
