@@ -125,6 +125,30 @@ GCM_API int gcm_measure_pipe_rates(double *rates, int n);
 #define GCM_PHASE_SLOTS 8
 GCM_API int gcm_set_phase_stamps(gcm_ctx *ctx, void *d_stamps);
 
+/*
+ * Diagnostics for the host logic (no CUDA call, usable without a GPU): the launch layout the library derives from
+ * the lengths of a message, and the chunk plan of the host-buffer pipeline.  Tests check their invariants and model
+ * the kernels' GHASH regrouping on the CPU from them.
+ *   gcm_debug_row_layout: virtual block sequence [pad | AAD | payload | length block] of one launch;
+ *     ctr_base = index of the launch's first payload block within its message, last = the launch ends the message,
+ *     aligned = the buffers are 16-byte aligned.  Returns GCM_OK / GCM_ERR_ARG / GCM_ERR_LEN.
+ *   gcm_debug_plan_chunks: chunk lengths of gcm_encrypt_host for a message of `len` bytes into plan[0 .. cap);
+ *     returns the number of chunks, or GCM_ERR_ARG when cap is too small.
+ */
+typedef struct {
+    uint64_t vblocks;        /* E: pad + AAD blocks + payload blocks + length block                         */
+    uint64_t base;           /* virtual index of payload block 0                                            */
+    uint32_t pad;            /* leading zero blocks, 0..31                                                   */
+    uint32_t n_aad_blocks;
+    uint32_t rows;           /* ceil(E / 32)                                                                 */
+    uint32_t fast_lo, fast_hi; /* rows [fast_lo, fast_hi) hold only whole payload blocks                     */
+    uint32_t ctr_delta;      /* counter of virtual block v = (uint32)v + ctr_delta                           */
+    uint32_t len_block;      /* 1: the last virtual block is the length block                                */
+    uint32_t reserved;
+} gcm_row_layout;
+GCM_API int gcm_debug_row_layout(uint64_t len, uint64_t aad_len, uint32_t ctr_base, int last, int aligned, gcm_row_layout *out);
+GCM_API int gcm_debug_plan_chunks(uint64_t len, uint64_t *plan, uint32_t cap);
+
 /* Copies the hash subkey H = E_K(0^128) (16 bytes) to host memory; for tests of step a2. */
 GCM_API int gcm_get_hash_subkey(const gcm_ctx *ctx, uint8_t h[16]);
 

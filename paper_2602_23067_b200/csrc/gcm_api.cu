@@ -286,6 +286,23 @@ extern "C" int gcm_get_hash_subkey(const gcm_ctx *c, uint8_t h[16])
     return GCM_OK;
 }
 
+extern "C" int gcm_debug_row_layout(uint64_t len, uint64_t aad_len, uint32_t ctr_base, int last, int aligned, gcm_row_layout *out)
+{
+    if (!out) return GCM_ERR_ARG;
+    if (len > ((1ull << 36) - 32) || aad_len >= (1ull << 61) || (aad_len + 15) / 16 > 0xFFFFFFFFull) return GCM_ERR_LEN;
+    RowMsg m;
+    memset(&m, 0, sizeof(m));
+    // only the alignment of the pointers matters to the layout
+    const uint8_t *fake = (const uint8_t *)(uintptr_t)(aligned ? 0x1000 : 0x1001);
+    row_msg_fill(m, fake, (uint8_t *)(uintptr_t)fake, fake, len, aad_len, ctr_base, last ? 1u : 0u, len, aad_len, false);
+    if (m.vblocks >= GCM_MAX_VBLOCKS) return GCM_ERR_LEN;
+    memset(out, 0, sizeof(*out));
+    out->vblocks = m.vblocks; out->base = m.base; out->pad = m.pad; out->n_aad_blocks = m.n_aad_blocks;
+    out->rows = m.rows; out->fast_lo = m.fast_lo; out->fast_hi = m.fast_hi; out->ctr_delta = m.ctr_delta;
+    out->len_block = m.len_block;
+    return GCM_OK;
+}
+
 extern "C" int gcm_set_phase_stamps(gcm_ctx *c, void *d_stamps)
 {
     if (!c) return GCM_ERR_ARG;

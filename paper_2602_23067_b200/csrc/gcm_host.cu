@@ -76,9 +76,9 @@ __global__ void gcm_chunk_pow_kernel(const uint4 *hx, const uint64_t *e, uint32_
 // with both directions busy every copy costs about 30 us on top of its bytes at 50 GB/s (a 4 MiB copy takes 113 us,
 // not 84), so the plan wants FEW chunks, while the first upload and the last download, which overlap with nothing,
 // want SMALL ones.  Hence: PIPE_MIN_CHUNK_BYTES at both ends, doubling up to the middle size (about len / 4, at most
-// PIPE_CHUNK_BYTES) and coming down again by a factor of about 0.6, slowly enough that a chunk's download is over
-// before the upload two chunks later wants its slot (s_k <= s_(k+1) + s_(k+2)).  Every chunk but the last is a
-// multiple of PIPE_MIN_CHUNK_BYTES (so of 16); the last one takes the ragged end.
+// PIPE_CHUNK_BYTES) and coming down again by a factor of about 0.6 per chunk (a chunk's slot is wanted again three
+// chunks later, so the sizes must not fall faster than the downloads drain).  Every chunk but the last is a multiple
+// of PIPE_MIN_CHUNK_BYTES (so of 16); the last one takes the ragged end.
 static uint32_t plan_chunks(uint64_t len, uint64_t *plan)
 {
     if (len == 0) { plan[0] = 0; return 1; }
@@ -287,6 +287,16 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
     if (!lock__.ok) return GCM_ERR_BUSY;                                                           \
     DeviceGuard guard__((c)->device);                                                              \
     CU(guard__.err)
+
+extern "C" int gcm_debug_plan_chunks(uint64_t len, uint64_t *plan, uint32_t cap)
+{
+    if (!plan || len > ((1ull << 36) - 32)) return GCM_ERR_ARG;
+    uint64_t full[PIPE_MAX_CHUNKS];
+    const uint32_t n = plan_chunks(len, full);
+    if (n > cap) return GCM_ERR_ARG;
+    memcpy(plan, full, n * sizeof(uint64_t));
+    return (int)n;
+}
 
 extern "C" int gcm_encrypt_host(gcm_ctx *c, const uint8_t iv[12], const void *h_aad, uint64_t aad_len,
                                 const void *h_pt, uint64_t len, void *h_ct, uint8_t tag[16], void *stream)

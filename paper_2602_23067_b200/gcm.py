@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = [
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
     "gcm_encrypt_host", "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
-    "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device",
+    "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_debug_row_layout", "gcm_debug_plan_chunks",
     "gcm_measure_pipe_rates",
 ]
 RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad"]
@@ -36,6 +36,14 @@ class GcmError(RuntimeError):
         if code == GCM_ERR_CUDA:
             detail = ": " + gcm_last_cuda_error_string()
         super().__init__("%s failed with code %d%s" % (where, code, detail))
+
+
+class GcmRowLayout(ctypes.Structure):
+    """struct gcm_row_layout of include/gcm.h"""
+    _fields_ = [("vblocks", ctypes.c_uint64), ("base", ctypes.c_uint64), ("pad", ctypes.c_uint32),
+                ("n_aad_blocks", ctypes.c_uint32), ("rows", ctypes.c_uint32), ("fast_lo", ctypes.c_uint32),
+                ("fast_hi", ctypes.c_uint32), ("ctr_delta", ctypes.c_uint32), ("len_block", ctypes.c_uint32),
+                ("reserved", ctypes.c_uint32)]
 
 
 class GcmMsg(ctypes.Structure):
@@ -90,6 +98,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_decrypt_verify_batch.argtypes = [ctypes.POINTER(GcmMsg), ctypes.c_uint32, vp]
     L.gcm_encrypt_batch_device.argtypes = [vp, ctypes.c_uint32, vp]
     L.gcm_decrypt_verify_batch_device.argtypes = [vp, ctypes.c_uint32, vp]
+    L.gcm_debug_row_layout.argtypes = [u64, u64, ctypes.c_uint32, ci, ci, ctypes.POINTER(GcmRowLayout)]
+    L.gcm_debug_plan_chunks.argtypes = [u64, ctypes.POINTER(u64), ctypes.c_uint32]
     L.gcm_batch_release.argtypes = []
     L.gcm_batch_release.restype = None
     L.gcm_measure_pipe_rates.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
@@ -423,6 +433,22 @@ def gcm_encrypt_batch_device(d_msgs, n: Optional[int] = None, stream=None) -> No
 def gcm_decrypt_verify_batch_device(d_msgs, n: Optional[int] = None, stream=None) -> None:
     ptr, n = _dmsgs(d_msgs, n)
     _check(_L.gcm_decrypt_verify_batch_device(ptr, n, _stream(stream)), "gcm_decrypt_verify_batch_device")
+
+
+def gcm_debug_row_layout(length: int, aad_len: int, ctr_base: int = 0, last: bool = True, aligned: bool = True) -> dict:
+    out = GcmRowLayout()
+    _check(_L.gcm_debug_row_layout(length, aad_len, ctr_base, 1 if last else 0, 1 if aligned else 0, ctypes.byref(out)),
+           "gcm_debug_row_layout")
+    return {k: getattr(out, k) for k, _ in GcmRowLayout._fields_ if k != "reserved"}
+
+
+def gcm_debug_plan_chunks(length: int) -> List[int]:
+    cap = 1200
+    plan = (ctypes.c_uint64 * cap)()
+    n = _L.gcm_debug_plan_chunks(length, plan, cap)
+    if n < 0:
+        raise GcmError(n, "gcm_debug_plan_chunks")
+    return [int(plan[i]) for i in range(n)]
 
 
 def gcm_batch_release() -> None:
