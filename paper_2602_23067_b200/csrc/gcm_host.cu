@@ -35,6 +35,9 @@ static cudaEvent_t dbg_ev[64][4];
 #ifndef PIPE_MIN_CHUNK_BYTES
 #define PIPE_MIN_CHUNK_BYTES (2ull << 20)   /* first and last chunk: what the pipeline cannot overlap */
 #endif
+#ifndef PIPE_ZEROCOPY_MAX_BYTES
+#define PIPE_ZEROCOPY_MAX_BYTES (4ull << 20)   /* up to here a pinned message is read and written in place over PCIe */
+#endif
 #define PIPE_MAX_CHUNKS ((uint32_t)((1ull << 36) / PIPE_CHUNK_BYTES) + 76)   /* 2^36 bytes in full chunks + the two ramps */
 
 struct HostPipe {
@@ -189,6 +192,39 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
 #ifdef GCM_PIPE_DEBUG
     const auto t_begin = std::chrono::steady_clock::now();
 #endif
+
+    // Short messages in pinned (or registered) host memory skip the staging copies altogether: under unified
+    // addressing the kernel reads the plaintext and writes the ciphertext in place over PCIe, one launch, no DMA
+    // set-up (measured on the B200 box: 1 MiB 57 us against 81 us staged; equal at 16 MiB; beyond that the copy
+    // engines win: kernel loads and stores together reach 30 GB/s, the two copy engines 2 x 50).
+    if (len > 0 && len <= PIPE_ZEROCOPY_MAX_BYTES && mode != MODE_GHASH && d_sum32 == nullptr) {
+        cudaPointerAttributes ai, ao;
+        if (cudaPointerGetAttributes(&ai, h_in) == cudaSuccess && cudaPointerGetAttributes(&ao, h_out) == cudaSuccess &&
+            ai.type == cudaMemoryTypeHost && ao.type == cudaMemoryTypeHost && ai.devicePointer && ao.devicePointer) {
+            cudaStream_t s0 = hp->stream[0];
+            CU(cudaEventRecord(hp->start, us));
+            CU(cudaStreamWaitEvent(s0, hp->start, 0));
+            if (aad_len) CU(cudaMemcpyAsync(hp->d_aad, h_aad, aad_len, cudaMemcpyHostToDevice, s0));
+            GcmParams p;
+            int blocks = 0;
+            rc = gcm_build_params(c, mode, iv, aad_len ? hp->d_aad : nullptr, aad_len, ai.devicePointer, len, ao.devicePointer,
+                                  0, true, len, aad_len, &p, &blocks);
+            if (rc != GCM_OK) return rc;
+            if (mode == MODE_DECRYPT) memcpy(p.tag_expect, tag_io, 16);
+            volatile int *verdict0 = (volatile int *)(c->h_pinned + 16);
+            *verdict0 = GCM_STATUS_PENDING;
+            p.tag_out = (uint4 *)c->h_pinned;
+            p.status = (int *)(c->h_pinned + 16);
+            cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s0);
+            memset(&p, 0, sizeof(p));
+            if (e != cudaSuccess) return gcm_cuda_fail(e);
+            CU(cudaStreamSynchronize(s0));
+            if (mode == MODE_ENCRYPT) { memcpy(tag_io, c->h_pinned, 16); return GCM_OK; }
+            if (*verdict0 != 0) { memset(h_out, 0, len); return GCM_ERR_AUTH; }
+            return GCM_OK;
+        }
+        cudaGetLastError();          // pageable memory: cudaPointerGetAttributes may leave an error behind on old drivers
+    }
 
     // chunk plan: small chunks at both ends, PIPE_CHUNK_BYTES in the middle
     uint64_t plan[PIPE_MAX_CHUNKS];
