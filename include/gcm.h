@@ -203,7 +203,7 @@ GCM_API int gcm_decrypt_verify_async(gcm_ctx *ctx, const uint8_t iv[12],
  * Host-buffer forms (the paper's data plane stages files through pinned host memory and overlaps
  * the transfers with the kernels on CUDA streams): `h_*` are HOST
  * pointers (pinned memory gives full PCIe rate; pageable memory works).  The message is cut into
- * chunks (about eight per message, 4 MiB to 64 MiB each) that travel H2D -> fused kernel -> D2H on three internal
+ * chunks (2 MiB at both ends of the message, doubling to at most 64 MiB in the middle) that travel H2D -> fused kernel -> D2H on three internal
  * streams; the running GHASH state is handed from chunk to chunk on the device.  The plaintext of chunk k is copied
  * out before the tag of the whole message is known (reading S9); gcm_decrypt_verify_host_strict does not do that.  Work already queued on `cuda_stream`
  * is waited for; the call returns when the output and the tag / verdict are in host memory.

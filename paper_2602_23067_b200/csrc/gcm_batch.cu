@@ -8,12 +8,15 @@
 //       the hash key H^(2^0), H^(2^1), ..."), and a 4-bit Shoup table of K = H^32 in the warp's own
 //       8 KB of shared memory (512 entries: cheap enough to build per message, unlike the 8-bit one)
 //   a3  E_K(J0) next to H (lane 0 encrypts 0^128, lane 1 encrypts J0)
-//   a4-a7  rows of 32 blocks exactly as in the fused kernel: cached counter rounds, T-table rounds,
-//       XOR, Y <- Y.K xor X with the ciphertext still in registers
+//   a4-a7, a10  the row loop shared with the fused kernel (gcm_device.cuh: gcm_rows): cached counter rounds,
+//       T-table rounds, XOR, Y <- Y.K xor X with the ciphertext still in registers, the length block as the
+//       last virtual block
 //   a8  the paper's binary tree (Fig. 3b) across the 32 lanes: at level k the left
-//       partial is multiplied by H^(2^k) and XORed into the right one
-//   a10-a11  length block, tag, constant-time compare, zero-fill of the output on mismatch.
-// Keys never touch global memory except inside the descriptor array, which is wiped after the call.
+//       partial is multiplied by H^(2^k) and XORed into the right one; one more product by H
+//   a11  tag, constant-time compare, zero-fill of the output on mismatch.
+// Host-descriptor calls (gcm_encrypt_batch / gcm_decrypt_verify_batch): keys never touch global memory except inside
+// the descriptor staging, which is wiped after the call.  Device-descriptor calls (gcm_*_batch_device): the caller's
+// own gcm_dmsg array is the descriptor array, a kernel orders the tickets, results go into the descriptors.
 //
 // Large messages (>= BATCH_LARGE_BYTES: FITS-sized HDUs, config C3) are grouped by key and go through
 // gcm_multi_kernel (gcm_multi.cu), ONE launch per key with a per-key context that is cached across calls; tags and
