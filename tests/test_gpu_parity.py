@@ -536,3 +536,59 @@ def test_host_pipeline_chunk_plan_boundaries(G, oracle):
             assert not bool(back.any().item())
     finally:
         G.gcm_destroy(ctx)
+
+
+def test_random_shapes_against_the_oracle(G, oracle):
+    """Differential run over 240 seeded random shapes: length (skewed towards row and block edges), AAD length,
+    key size, source / destination / AAD misalignment, in place or not, launch geometry (threads 256 / 384 / 512, 1-300
+    CTAs, or the default with its latency-kernel switch), encrypt then decrypt_verify, every byte and tag against the
+    oracle, nothing written outside the output range."""
+    rng = np.random.default_rng(9990)
+    ctxs = {}
+    try:
+        for case in range(240):
+            klen = 16 if rng.integers(0, 2) else 32
+            key = ctxs.get(klen)
+            if key is None:
+                k = rnd(rng, klen).tobytes()
+                ctxs[klen] = key = (k, G.gcm_init(k))
+            k, ctx = key
+            kind = int(rng.integers(0, 4))
+            if kind == 0:
+                n = int(rng.integers(0, 600))
+            elif kind == 1:
+                n = 512 * int(rng.integers(1, 40)) + int(rng.integers(-17, 18))
+            elif kind == 2:
+                n = 16 * int(rng.integers(1, 20000)) + int(rng.integers(0, 16))
+            else:
+                n = int(rng.integers(1, 1 << 20))
+            n = max(n, 0)
+            a = int(rng.choice([0, 0, 1, 15, 16, 17, 45, 256, 2880, int(rng.integers(0, 4000))]))
+            oi, oo, oa = (int(rng.integers(0, 16)) if rng.integers(0, 3) == 0 else 0 for _ in range(3))
+            in_place = bool(rng.integers(0, 4) == 0)
+            geom = [(0, 0), (0, 0), (1, 256), (3, 384), (7, 512), (148, 384), (int(rng.integers(1, 300)), int(rng.choice([256, 384, 512])))][int(rng.integers(0, 7))]
+            G.gcm_set_geometry(ctx, *geom)
+            iv, aad, pt = rnd(rng, 12).tobytes(), rnd(rng, a), rnd(rng, n)
+            ref_ct, ref_tag = oracle.gcm_encrypt(k, iv, aad, pt)
+            big_in = torch.zeros(n + 48, dtype=torch.uint8, device="cuda")
+            big_in[oi: oi + n] = dev(pt)
+            big_aad = torch.zeros(a + 32, dtype=torch.uint8, device="cuda")
+            big_aad[oa: oa + a] = dev(aad)
+            if in_place:
+                big_out, oo = big_in, oi
+            else:
+                big_out = torch.zeros(n + 48, dtype=torch.uint8, device="cuda")
+            d_aad = big_aad[oa: oa + a] if a else None
+            tag = G.gcm_encrypt(ctx, iv, d_aad, big_in[oi: oi + n], big_out[oo: oo + n])
+            out = big_out.cpu().numpy()
+            note = (case, klen, n, a, oi, oo, oa, in_place, geom)
+            assert tag == ref_tag, note
+            assert np.array_equal(out[oo: oo + n], ref_ct), note
+            assert not out[:oo].any() and not out[oo + n:].any(), note
+            back = torch.full((n + 32,), 0x5C, dtype=torch.uint8, device="cuda")
+            assert G.gcm_decrypt_verify(ctx, iv, d_aad, big_out[oo: oo + n], back[16: 16 + n], tag) == G.GCM_OK, note
+            got = back.cpu().numpy()
+            assert np.array_equal(got[16: 16 + n], pt) and (got[:16] == 0x5C).all() and (got[16 + n:] == 0x5C).all(), note
+    finally:
+        for _, ctx in ctxs.values():
+            G.gcm_destroy(ctx)
