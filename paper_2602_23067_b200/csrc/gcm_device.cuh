@@ -339,19 +339,21 @@ struct MulK8 {                 // 8-bit Shoup table of K in shared memory at KTA
 
 // ---- the row loop: SURVEY.md 8(a) a4-a7 for rows [r0, r1) of one message ------------------------------------
 // MSG: accessor view of a RowMsg (hot fields in registers or constant bank, cold ones wherever they live).
-// RK:  indexable round keys.  MUL: y -> y . K.  Returns the lane's running value Y (a7) after its last block.
+// RK:  indexable round keys.  GH: the GHASH leaf fold (a7): gh.pre() before a row's AES, gh.absorb(X, take) with the
+// row's GHASH input block after it (take = false: the lane has no block in this row).  TableGhash (below) multiplies
+// by K through a shared-memory table (MUL: y -> y . K) and gcm_rows() returns its running value Y after the last
+// block; TensorGhash (gcm_tc.cu) hands the blocks to the tensor core.
 // The same code serves the single-message kernel (gcm_fused.cu), the many-large-messages kernel (gcm_multi.cu)
 // and the warp-per-message kernel (gcm_batch.cu).
 // DEPTH: rows of payload a lane keeps in flight ahead of the one it works on.  One row (512 B per warp, 8 KB per
 // SM) covers the 1 TB/s the AES modes read; GHASH-only reads twice as fast and needs more bytes in flight to
 // cover the HBM latency (Little's law: 2 TB/s x 0.8 us = 11 KB per SM).
-template <int NR, int MODE, int DEPTH = 1, class MSG, class RK, class MUL>
-__device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint8_t *sm, uint32_t lane,
-                                          const CtrConst &cc, uint32_t r0, uint32_t r1, const MUL &mul)
+template <int NR, int MODE, int DEPTH = 1, class MSG, class RK, class GH>
+__device__ __forceinline__ void gcm_rows_gh(const MSG &m, const RK &rk, const uint8_t *sm, uint32_t lane,
+                                            const CtrConst &cc, uint32_t r0, uint32_t r1, GH &gh)
 {
     const uint32_t lane4 = lane * 4;
     CtrCache cu = {0, 0, 0, 0};
-    uint4 Y = make_uint4(0, 0, 0, 0);
     uint4 pre = make_uint4(0, 0, 0, 0);
     bool have_pre = false;
     const uint32_t first_fast = r0 > m.fast_lo() ? r0 : m.fast_lo();      // first fast row of this run (if any)
@@ -373,12 +375,13 @@ __device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint
                 for (int k = 0; k < DEPTH; k++) {
                     const uint4 xk = buf[k];
                     if (i + DEPTH + k < n) buf[k] = ld16_stream(src + 512ull * (i + DEPTH + k));
-                    Y = xor4(mul(Y), xk);
+                    gh.pre();
+                    gh.absorb(xk, true);
                 }
             }
 #pragma unroll
             for (int k = 0; k < DEPTH; k++)
-                if (i + k < n) Y = xor4(mul(Y), buf[k]);
+                if (i + k < n) { gh.pre(); gh.absorb(buf[k], true); }
             row = lim - 1;
             continue;
         }
@@ -413,7 +416,7 @@ __device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint
             }
         }
         // a7: multiply the running value by K; independent of this row's AES, so they interleave
-        const uint4 ym = mul(Y);
+        gh.pre();
         uint4 X = x;
         if (MODE != MODE_GHASH) {
             // a4: counter from the virtual index alone; the upper 24 bits are warp-uniform and change
@@ -426,9 +429,27 @@ __device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint
             else if (cbytes) store_bytes(m.out() + 16 * g, y, cbytes);
             if (MODE == MODE_ENCRYPT && cbytes) X = keep_bytes(y, cbytes);
         }
-        if (fast || valid) Y = xor4(ym, X);
+        gh.absorb(X, fast || valid);
     }
-    return Y;
+}
+
+// GH for a table multiplier: Y <- Y.K xor X, the product formed ahead of the row's AES.
+template <class MUL>
+struct TableGhash {
+    const MUL &mul;
+    uint4 Y, ym;
+    __device__ __forceinline__ explicit TableGhash(const MUL &mul_, uint4 y0 = make_uint4(0, 0, 0, 0)) : mul(mul_), Y(y0), ym(y0) {}
+    __device__ __forceinline__ void pre() { ym = mul(Y); }
+    __device__ __forceinline__ void absorb(uint4 X, bool take) { if (take) Y = xor4(ym, X); }
+};
+
+template <int NR, int MODE, int DEPTH = 1, class MSG, class RK, class MUL>
+__device__ __forceinline__ uint4 gcm_rows(const MSG &m, const RK &rk, const uint8_t *sm, uint32_t lane,
+                                          const CtrConst &cc, uint32_t r0, uint32_t r1, const MUL &mul)
+{
+    TableGhash<MUL> gh(mul);
+    gcm_rows_gh<NR, MODE, DEPTH>(m, rk, sm, lane, cc, r0, r1, gh);
+    return gh.Y;
 }
 
 // Exponent (1..32) of the power of H that aligns lane `lane`'s running value with the end of its run of rows:
