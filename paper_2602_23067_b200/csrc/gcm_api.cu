@@ -15,6 +15,7 @@
 #include "gcm_common.cuh"
 #include "gcm_setup.cuh"
 #include "gcm_fused.cuh"
+#include "gcm_tc.cuh"
 #include "gcm_api_internal.h"
 
 // Device for new contexts: -1 = the calling thread's current CUDA device, else the ordinal given to gcm_set_device.
@@ -168,7 +169,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     size_t o_te0 = take(256 * 4), o_rk = take(64 * 4), o_h = take(16);
     size_t o_hpow = take((GCM_STRIDE + 1) * 16), o_hx = take(HX_ENTRIES * 16);
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
-    size_t o_cnt = take(4), o_tag = take(16), o_status = take(4);
+    size_t o_cnt = take(4), o_tag = take(16), o_status = take(4), o_bmat = take(TC_BMAT_TOTAL);
     c->slab_bytes = off;
     cudaError_t e = cudaSuccess;
     {
@@ -192,6 +193,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     c->d_counter = (unsigned *)(c->d_slab + o_cnt);
     c->d_tag = (uint4 *)(c->d_slab + o_tag);
     c->d_status = (int *)(c->d_slab + o_status);
+    c->d_bmat = (uint4 *)(c->d_slab + o_bmat);
 
     int rc = GCM_OK;
     do {
@@ -200,6 +202,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
         SetupParams sp = setup_params(c, key);
         launch_setup(sp, 0);
         secure_zero(&sp, sizeof(sp));
+        launch_tc_setup(c->d_hx, c->d_bmat, 0);        // a2 for the tensor-core GHASH: bit matrices of K^0 .. K^TC_L
         if ((e = cudaGetLastError()) != cudaSuccess) break;
         // synchronous copy: the tables are complete before any kernel of this context can be launched (the
         // fused kernel reads them ahead of griddepcontrol.wait and relies on that)
@@ -269,6 +272,20 @@ extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)
     return GCM_OK;
 }
 
+extern "C" int gcm_set_ghash_engine(gcm_ctx *c, int engine)
+{
+    if (!c || (engine != GCM_GHASH_TABLE && engine != GCM_GHASH_TENSOR)) return GCM_ERR_ARG;
+    c->engine = engine;
+    return GCM_OK;
+}
+
+extern "C" int gcm_get_ghash_engine(const gcm_ctx *c, int *engine)
+{
+    if (!c || !engine) return GCM_ERR_ARG;
+    *engine = c->engine;
+    return GCM_OK;
+}
+
 extern "C" int gcm_get_geometry(const gcm_ctx *c, int *grid, int *threads)
 {
     if (!c) return GCM_ERR_ARG;
@@ -334,7 +351,7 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     // rows are dealt to the warps of the grid in contiguous runs balanced to +-1 row; a short message uses
     // only as many CTAs as it has rows for
     const uint64_t S = p->m.rows;
-    const uint64_t wpc = (uint64_t)c->threads / 32;              // warps per CTA
+    const uint64_t wpc = c->engine == GCM_GHASH_TENSOR ? TC_PRODUCER_WARPS : (uint64_t)c->threads / 32;   // warps per CTA that take rows
     uint64_t want = (S + wpc - 1) / wpc;
     if (want < 1) want = 1;
     if (want > (uint64_t)c->grid) want = (uint64_t)c->grid;
@@ -345,6 +362,7 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
     p->tab.hpow = c->d_hpow;
     p->tab.hx = c->d_hx;
     p->tab.h = c->d_h;
+    p->tab.bmat = c->d_bmat;
     p->partials = c->d_partials;
     p->counter = c->d_counter;
     c->ticket_next += (unsigned)want;                            // epoch scheme: see GcmParams::ticket_last
@@ -359,7 +377,8 @@ int gcm_build_params(gcm_ctx *c, int mode, const uint8_t *iv, const void *d_aad,
 // explicit gcm_set_geometry always selects the fused kernel (the geometry tests rely on that).
 cudaError_t gcm_launch_fused(gcm_ctx *c, int mode, int blocks, const GcmParams &p, cudaStream_t s)
 {
-    const cudaError_t e = launch_fused(c->nr, mode, c->threads, blocks, p, s);
+    const cudaError_t e = c->engine == GCM_GHASH_TENSOR ? launch_tc(c->nr, mode, blocks, p, s)
+                                                        : launch_fused(c->nr, mode, c->threads, blocks, p, s);
     if (e != cudaSuccess) c->ticket_next -= (unsigned)blocks;    // the launch was not made: its tickets are not drawn
     return e;
 }

@@ -13,6 +13,7 @@ struct gcm_ctx {
     int sm_count;
     int grid;          // CTAs of the fused kernel at most (default: one per SM)
     int threads;       // threads per CTA (512 default, 256 / 384 alternatives)
+    int engine;        // GCM_GHASH_TABLE / GCM_GHASH_TENSOR: which single-message kernel multiplies by K (gcm_set_ghash_engine)
     // device state, one slab
     uint8_t  *d_slab;
     size_t    slab_bytes;
@@ -22,6 +23,7 @@ struct gcm_ctx {
     uint4    *d_hpow;
     uint4    *d_hx;
     uint4    *d_ktab;
+    uint4    *d_bmat;     // bit matrices of K^0 .. K^TC_L (gcm_tc.cu)
     uint4    *d_partials;
     unsigned *d_counter;
     uint4    *d_tag;

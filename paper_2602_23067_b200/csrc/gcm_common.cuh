@@ -28,6 +28,14 @@
 #define MBAR_OFF        (WPOW_OFF + WPOW_BYTES)     /* one mbarrier (8 B) for the bulk copy of ktab */
 #define FUSED_SMEM_BYTES (MBAR_OFF + 16)
 
+// ---- GHASH on the tensor cores (gcm_tc.cu) ------------------------------------------------------
+// A lane's TC_L consecutive blocks and its running value make one chunk = TC_L + 1 slices of one tcgen05.mma tile;
+// slice weights are K^0 .. K^TC_L (K = H^32), one 8 KB bit matrix each (the MMA's B operand, in shared memory).
+#define TC_L              8
+#define TC_BMAT_BYTES     8192
+#define TC_BMAT_TOTAL     ((TC_L + 1) * TC_BMAT_BYTES)
+#define TC_PRODUCER_WARPS 12          /* + one warp that issues the MMAs: 416 threads per CTA */
+
 #define GCM_MAX_THREADS 512
 #define GCM_MAX_GRID    4096
 #define GCM_MAX_DEVICES 64
@@ -49,6 +57,7 @@ struct GcmTables {
     const uint4    *hpow;    // hpow[i] = H^i, i = 0..GCM_STRIDE ("mem" format)
     const uint4    *hx;      // HX_ENTRIES radix-512 powers
     const uint4    *h;       // H
+    const uint4    *bmat;    // TC_BMAT_TOTAL: bit matrices of K^0 .. K^TC_L for the tensor-core GHASH (gcm_tc.cu)
 };
 
 // One message as the row loop (gcm_device.cuh: gcm_rows) sees it.

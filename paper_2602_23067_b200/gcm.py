@@ -13,13 +13,15 @@ from typing import Iterable, List, Optional, Sequence, Tuple
 
 GCM_OK, GCM_ERR_AUTH, GCM_ERR_ARG, GCM_ERR_LEN, GCM_ERR_CUDA, GCM_ERR_NOMEM, GCM_ERR_BUSY = 0, 1, -1, -2, -3, -4, -5
 GCM_PHASE_SLOTS = 8
+GCM_GHASH_TABLE = 0
+GCM_GHASH_TENSOR = 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libb200gcm.so")
 
 EXPORTED_SYMBOLS = [
     "gcm_version", "gcm_set_device", "gcm_last_cuda_error", "gcm_last_cuda_error_string",
-    "gcm_init", "gcm_destroy", "gcm_set_geometry", "gcm_get_geometry", "gcm_get_hash_subkey",
+    "gcm_init", "gcm_destroy", "gcm_set_geometry", "gcm_get_geometry", "gcm_set_ghash_engine", "gcm_get_ghash_engine", "gcm_get_hash_subkey",
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
     "gcm_encrypt_host", "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
@@ -84,6 +86,8 @@ def _load() -> ctypes.CDLL:
     L.gcm_destroy.restype = None
     L.gcm_set_geometry.argtypes = [vp, ci, ci]
     L.gcm_get_geometry.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci)]
+    L.gcm_set_ghash_engine.argtypes = [vp, ci]
+    L.gcm_get_ghash_engine.argtypes = [vp, ctypes.POINTER(ci)]
     L.gcm_get_hash_subkey.argtypes = [vp, ctypes.c_char_p]
     L.gcm_encrypt.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
     L.gcm_decrypt_verify.argtypes = [vp, ctypes.c_char_p, vp, u64, vp, u64, vp, ctypes.c_char_p, vp]
@@ -198,6 +202,16 @@ def gcm_get_geometry(ctx: int) -> Tuple[int, int]:
     g, t = ctypes.c_int(), ctypes.c_int()
     _check(_L.gcm_get_geometry(ctx, ctypes.byref(g), ctypes.byref(t)), "gcm_get_geometry")
     return g.value, t.value
+
+
+def gcm_set_ghash_engine(ctx: int, engine: int) -> None:
+    _check(_L.gcm_set_ghash_engine(ctx, int(engine)), "gcm_set_ghash_engine")
+
+
+def gcm_get_ghash_engine(ctx: int) -> int:
+    e = ctypes.c_int()
+    _check(_L.gcm_get_ghash_engine(ctx, ctypes.byref(e)), "gcm_get_ghash_engine")
+    return e.value
 
 
 def gcm_get_hash_subkey(ctx: int) -> bytes:
@@ -488,6 +502,9 @@ class Context:
 
     def set_geometry(self, grid: int = 0, threads: int = 0) -> None:
         gcm_set_geometry(self.handle, grid, threads)
+
+    def set_ghash_engine(self, engine: int) -> None:
+        gcm_set_ghash_engine(self.handle, engine)
 
     def encrypt(self, iv, aad, pt, ct=None, stream=None):
         import torch
