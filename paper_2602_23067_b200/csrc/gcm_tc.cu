@@ -28,11 +28,11 @@
 //     first slice of the next chunk.  At the end of the run Y is exactly what the table recurrence would have left,
 //     and the epilogue of gcm_fused.cu (lane exponent, warp XOR, position weights, last-CTA-done) follows unchanged.
 //
-// Roles: 12 producer warps in 3 groups of 4 (warp & 3 selects the TMEM lane quarter a warp may touch) + 1 warp whose
-// lane 0 issues every tcgen05.mma.  Per group: one accumulator (128 columns), a ring of two A slices (16 columns
+// Roles: 12 producer warps in 3 groups of 4 (warp & 3 selects the TMEM lane quarter a warp may touch) + 3 warps whose
+// lane 0 issues the tcgen05.mma of one group each (the groups do not wait for one another).  Per group: one accumulator (128 columns), a ring of two A slices (16 columns
 // each), mbarriers full[2] (4 producer arrivals), empty[2] and accfull (tcgen05.commit).  Every warp of the CTA runs
 // the same number of rows (a run that is one row short starts with an empty row: zero blocks are free in GHASH), so
-// the issuing lane walks slices and groups in a fixed order.
+// the issuing lanes know the slice sequence without being told.
 #include "gcm_common.cuh"
 #include "gf128.cuh"
 #include "gcm_fused.cuh"
@@ -43,7 +43,8 @@
 #include <atomic>
 
 #define TC_NW        12                              /* producer warps */
-#define TC_THREADS   (32 * (TC_NW + 1))
+#define TC_NG        (TC_NW / 4)                     /* groups = issuing warps */
+#define TC_THREADS   (32 * (TC_NW + TC_NG))
 #define TC_BMAT_OFF  AES_TAB_BYTES
 #define TC_RED_OFF   (TC_BMAT_OFF + TC_BMAT_TOTAL)
 #define TC_WPOW_OFF  (TC_RED_OFF + 512)
@@ -123,10 +124,11 @@ struct TensorGhash {
     uint32_t n;             // slices stored so far
     uint32_t in_chunk, ell, rows_left, chunk;
     bool pending;           // the last slice's tcgen05.st has not been waited for / announced yet
+    bool owed;              // a finished chunk's result has not been read back yet
     uint4 Y;
 
     __device__ __forceinline__ TensorGhash(uint32_t tbase, uint32_t warp, uint32_t lane_, uint64_t *bars, uint32_t rows)
-        : lane(lane_), n(0), in_chunk(0), chunk(0), pending(false), Y(make_uint4(0, 0, 0, 0))
+        : lane(lane_), n(0), in_chunk(0), chunk(0), pending(false), owed(false), Y(make_uint4(0, 0, 0, 0))
     {
         const uint32_t g = warp >> 2, q = warp & 3;
         lanebase = tbase + ((32u * q) << 16);
@@ -167,9 +169,10 @@ struct TensorGhash {
         pending = true;
         n++;
     }
-    __device__ __forceinline__ void end_chunk()
+    // The chunk's accumulator row -> Y (and on into the next chunk as its first slice).  Called one row AFTER the
+    // chunk's last slice was announced, i.e. behind the next row's AES: the MMAs have long finished by then.
+    __device__ __forceinline__ void extract()
     {
-        flush();
         mbar_wait(accfull, chunk & 1);
         tc_fence_after();
         uint32_t r[32];
@@ -178,17 +181,26 @@ struct TensorGhash {
         tc_ld32(lanebase + acc + 64, r); Y.z = tc_parity32(r);
         tc_ld32(lanebase + acc + 96, r); Y.w = tc_parity32(r);
         chunk++;
-        in_chunk = 0;
-        ell = rows_left < TC_L ? rows_left : TC_L;
-        if (rows_left) emit(Y);                                 // the running value leads the next chunk
+        owed = false;
     }
     __device__ __forceinline__ void pre() {}
     __device__ __forceinline__ void absorb(uint4 X, bool take)
     {
+        if (owed) { extract(); emit(Y); }                       // the running value leads the new chunk
         emit(take ? X : make_uint4(0, 0, 0, 0));
         in_chunk++;
         rows_left--;
-        if (in_chunk == ell) end_chunk();
+        if (in_chunk == ell) {                                  // chunk complete: announce its last slice now,
+            flush();                                            // read the result back later
+            owed = true;
+            in_chunk = 0;
+            ell = rows_left < TC_L ? rows_left : TC_L;
+        }
+    }
+    __device__ __forceinline__ uint4 finish()
+    {
+        if (owed) extract();
+        return Y;
     }
 };
 
@@ -266,7 +278,7 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
         __syncwarp();
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tslot)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    } else {
+    } else if (warp < TC_NW) {
         if (MODE != MODE_GHASH) fill_aes_tables<32 * TC_NW>(sm, p.te0, t);
         const uint64_t wg = (uint64_t)blockIdx.x * TC_NW + warp;
         r0 = __shfl_sync(0xFFFFFFFFu, (uint32_t)((wg * S) / p.warps), 0);
@@ -281,9 +293,11 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
     tc_fence_after();
     const uint32_t tbase = *tslot;
 
-    if (warp == TC_NW) {
-        // ---- the issuing lane: slices in order, groups round-robin --------------------------------------------
+    if (warp >= TC_NW) {
+        // ---- the issuing lane of group g: its slices in order -------------------------------------------------
         if (lane == 0) {
+            const uint32_t g = warp - TC_NW;
+            uint64_t *full = bars + 1 + 2 * g, *empty = bars + 7 + 2 * g;
             mbar_wait(bars + 0, 0);
             const uint32_t bm = smem_u32(sm + TC_BMAT_OFF), sf = tbase + TC_COL_SF;
             uint32_t n = 0, left = rmax;
@@ -296,17 +310,13 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
                     const uint32_t slot = n & 1;
                     const uint64_t b0 = tc_smem_desc(bm + e * TC_BMAT_BYTES, 2048, 128);
                     const uint64_t b1 = tc_smem_desc(bm + e * TC_BMAT_BYTES + 4096, 2048, 128);
-#pragma unroll
-                    for (uint32_t g = 0; g < 3; g++) {
-                        uint64_t *full = bars + 1 + 2 * g, *empty = bars + 7 + 2 * g;
-                        mbar_wait(full + slot, (n >> 1) & 1);
-                        tc_fence_after();
-                        const uint32_t a = tbase + TC_COL_RING + 32 * g + 16 * slot;
-                        tc_mma(tbase + 128 * g, a, b0, sf, j != 0);
-                        tc_mma(tbase + 128 * g, a + 8, b1, sf, 1);
-                        tc_commit(empty + slot);
-                        if (j + 1 == nsl) tc_commit(bars + 13 + g);
-                    }
+                    mbar_wait(full + slot, (n >> 1) & 1);
+                    tc_fence_after();
+                    const uint32_t a = tbase + TC_COL_RING + 32 * g + 16 * slot;
+                    tc_mma(tbase + 128 * g, a, b0, sf, j != 0);
+                    tc_mma(tbase + 128 * g, a + 8, b1, sf, 1);
+                    tc_commit(empty + slot);
+                    if (j + 1 == nsl) tc_commit(bars + 13 + g);
                 }
             }
         }
@@ -314,7 +324,7 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
         tc_fence_before();
         __syncthreads();                                // epilogue barrier of the producers: every tcgen05.ld is done
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase) : "memory");
+        if (warp == TC_NW) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase) : "memory");
         return;
     }
 
@@ -349,7 +359,7 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
     TensorGhash gh(tbase, warp, lane, bars, rmax);
     for (uint32_t k = rt - r0; k < rmax; k++) gh.absorb(make_uint4(0, 0, 0, 0), false);   // a run that is short starts with empty rows
     gcm_rows_gh<NR, MODE, MODE == MODE_GHASH ? 2 : 1>(m, p.rk, sm, lane, cc, r0, rt, gh);  // a4-a7
-    uint4 Y = gh.Y;
+    uint4 Y = gh.finish();
     if (rt < r1) {
         ProductGhash gl(__ldg(p.tab.hpow + GCM_STRIDE), Y);
         gcm_rows_gh<NR, MODE, 1>(m, p.rk, sm, lane, cc, rt, r1, gl);
