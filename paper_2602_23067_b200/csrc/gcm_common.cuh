@@ -36,6 +36,13 @@
 #define TC_BMAT_TOTAL     ((TC_L + 1) * TC_BMAT_BYTES)
 #define TC_PRODUCER_WARPS 12          /* + one warp that issues the MMAs: 416 threads per CTA */
 
+// GHASH-only on the tensor cores (gcm_ghash_tc.cu): chunks of GT_L slices of 128 consecutive blocks; slice weights are
+// powers of H^128, the chunk-to-chunk multiplier H^(128 GT_L) goes through an 8-bit table.
+#define GT_L              16
+#define GT_CHUNK_BLOCKS   (128 * GT_L)
+#define GT_BMAT_TOTAL     (GT_L * TC_BMAT_BYTES)
+#define GT_MIN_BYTES      (4ull << 20)   /* shorter messages stay with the row kernels */
+
 #define GCM_MAX_THREADS 512
 #define GCM_MAX_GRID    4096
 #define GCM_MAX_DEVICES 64
