@@ -46,6 +46,7 @@
 #define GT_IDESC ((1u << 7) | (1u << 10) | (16u << 17) | (1u << 23) | (8u << 24))
 static_assert(GT_RING % (GT_PRODUCERS / 4) == 0, "a warp's slices keep their ring phase");
 static_assert(GT_STAGES % (GT_PRODUCERS / 4) != 0 || true, "");
+static_assert(GT_RING % 4 == 0 && GT_L % 4 == 0, "the issue loop takes four slices per trip");
 static_assert(GT_BMAT_TOTAL == KTAB_OFF, "the matrices fill the 128 KB in front of the multiplier table");
 
 struct GhashTcParams {
@@ -261,26 +262,32 @@ gcm_ghash_tc_kernel(const __grid_constant__ GhashTcParams p)
         const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
         const uint64_t dtop = gt_smem_desc(smem_u32(sm + GT_BMAT_OFF) + (GT_L - 1) * TC_BMAT_BYTES, 2048, 128);   // matrix of K^(GT_L-1), first half
         const uint32_t dhi = (uint32_t)(dtop >> 32), dlo_top = (uint32_t)dtop;
-        uint32_t a = ring0, fa = full0, ea = empty0, slot = 0, ph = 0;
+        uint32_t slot0 = 0, ph0 = 0;                                   // ring position and phase at the start of the chunk
         for (uint32_t c = 0; c < nch; c++) {
             const uint32_t b = c & 1, d = tb + 128 * b;
             mbar_wait(accempty + b, ((c >> 1) & 1) ^ 1);               // the read-back of this buffer's previous chunk is done
-            uint32_t dlo = dlo_top;
+            if (gt_elect()) {
+                uint32_t dlo = dlo_top, slot = slot0, ph = ph0;
+                uint32_t a = ring0 + 16 * slot, fa = full0 + 8 * slot, ea = empty0 + 8 * slot;
 #pragma unroll 1
-            for (uint32_t s = 0; s < GT_L; s++) {
-                mbar_wait_addr(fa, ph);
-                gt_fence_after();
-                if (gt_elect()) {
-                    gt_mma(d, a, ((uint64_t)dhi << 32) | dlo, sf, s);
-                    gt_mma(d, a + 8, ((uint64_t)dhi << 32) | (dlo + 256), sf, 1);
-                    gt_commit_addr(ea);
-                    if (s == GT_L - 1) gt_commit(accfull + b);
+                for (uint32_t s = 0; s < GT_L; s += 4) {               // four slices per trip: offsets fold into the instructions
+#pragma unroll
+                    for (uint32_t k = 0; k < 4; k++) {
+                        mbar_wait_addr(fa + 8 * k, ph);
+                        gt_fence_after();
+                        gt_mma(d, a + 16 * k, ((uint64_t)dhi << 32) | (dlo - 512 * k), sf, s + k);
+                        gt_mma(d, a + 16 * k + 8, ((uint64_t)dhi << 32) | (dlo - 512 * k + 256), sf, 1);
+                        gt_commit_addr(ea + 8 * k);
+                    }
+                    dlo -= 4 * (TC_BMAT_BYTES >> 4);                   // on to the next lower powers of K
+                    a += 64; fa += 32; ea += 32; slot += 4;
+                    if (slot == GT_RING) { slot = 0; ph ^= 1; a = ring0; fa = full0; ea = empty0; }
                 }
-                __syncwarp();
-                dlo -= TC_BMAT_BYTES >> 4;                             // next slice: the next lower power of K
-                a += 16; fa += 8; ea += 8;
-                if (++slot == GT_RING) { slot = 0; ph ^= 1; a = ring0; fa = full0; ea = empty0; }
+                gt_commit(accfull + b);
             }
+            __syncwarp();
+            slot0 += GT_L;                                              // every lane keeps the chunk-level position
+            while (slot0 >= GT_RING) { slot0 -= GT_RING; ph0 ^= 1; }
         }
     } else {
         // ---- read-back warps: row 32 q + lane -----------------------------------------------------------------------
