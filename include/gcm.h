@@ -97,16 +97,21 @@ GCM_API int gcm_set_geometry(gcm_ctx *ctx, int grid, int threads);
 GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
 
 /*
- * Which unit multiplies the running GHASH value by the stride power K = H^32 in the single-message kernel (step a7 of
- * the path; Eq. 1 leaves the method of the GF(2^128) multiply open, reading S7):
- *   GCM_GHASH_TABLE   an 8-bit Shoup table in shared memory, 16 reads of 16 bytes per block (gcm_fused.cu);
+ * Which unit does the GF(2^128) multiplies of GHASH (step a7 of the path; Eq. 1 leaves the method
+ * of the multiply open, reading S7):
+ *   GCM_GHASH_TABLE   an 8-bit Shoup table of the stride power K = H^32 in shared memory, 16 reads of 16 bytes per
+ *                     block (gcm_fused.cu), for every call;
  *   GCM_GHASH_TENSOR  the tensor cores: the multiply as a GF(2) matrix-vector product, tcgen05.mma kind::mxf4 with
- *                     0 / 1 operands, accumulators in TMEM, parity of the counts (gcm_tc.cu).  Its CTAs have 12 warps
- *                     that take rows (+ 1 that issues the MMAs); `threads` of gcm_set_geometry is ignored, `grid` kept.
- * Results are bit-identical under both.  The batched calls and the latency kernel are not affected.
+ *                     0 / 1 operands, accumulators in TMEM, parity of the counts.  The single-message encrypt / decrypt /
+ *                     GHASH calls run gcm_tc.cu (CTAs of 12 warps that take rows + 3 that issue the MMAs; `threads` of
+ *                     gcm_set_geometry is ignored, `grid` kept), and gcm_ghash_async on at least 4 MiB of 16-byte
+ *                     aligned input runs gcm_ghash_tc.cu over the whole 32 KiB chunks of it;
+ *   GCM_GHASH_AUTO    (default) what is fastest on a B200: the table for encrypt / decrypt, the tensor cores for
+ *                     gcm_ghash_async on long aligned input.
+ * Results are bit-identical under all three.  The batched calls and the latency kernel are not affected.
  * Returns GCM_OK / GCM_ERR_ARG.
  */
-enum { GCM_GHASH_TABLE = 0, GCM_GHASH_TENSOR = 1 };
+enum { GCM_GHASH_TABLE = 0, GCM_GHASH_TENSOR = 1, GCM_GHASH_AUTO = 2 };
 GCM_API int gcm_set_ghash_engine(gcm_ctx *ctx, int engine);
 GCM_API int gcm_get_ghash_engine(const gcm_ctx *ctx, int *engine);
 

@@ -162,6 +162,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     c->sm_count = sm_count;
     c->grid = c->sm_count;
     c->threads = GCM_MAX_THREADS;
+    c->engine = GCM_GHASH_AUTO;
 
     // one slab for all device-side state
     size_t off = 0;
@@ -279,7 +280,7 @@ extern "C" int gcm_set_geometry(gcm_ctx *c, int grid, int threads)
 
 extern "C" int gcm_set_ghash_engine(gcm_ctx *c, int engine)
 {
-    if (!c || (engine != GCM_GHASH_TABLE && engine != GCM_GHASH_TENSOR)) return GCM_ERR_ARG;
+    if (!c || (engine != GCM_GHASH_TABLE && engine != GCM_GHASH_TENSOR && engine != GCM_GHASH_AUTO)) return GCM_ERR_ARG;
     c->engine = engine;
     return GCM_OK;
 }
@@ -466,6 +467,7 @@ static int ghash_tensor_locked(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
         if (rc != GCM_OK) return rc;
         p.chain_out = c->d_gt + 0;
         e = gcm_launch_fused(c, MODE_GHASH, blocks, p, s);
+        secure_zero(&p, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
     }
     const uint64_t tail = len - bulk;
@@ -480,6 +482,7 @@ static int ghash_tensor_locked(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     p.chain_pow = c->d_gt + 2;
     p.tag_out = (uint4 *)d_out;
     e = gcm_launch_fused(c, MODE_GHASH, blocks, p, s);
+    secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;
 }
@@ -491,7 +494,7 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     GcmParams p;
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
-    if (c->engine == GCM_GHASH_TENSOR && len >= GT_MIN_BYTES && d_c && ((uintptr_t)d_c & 15) == 0 &&
+    if (c->engine != GCM_GHASH_TABLE && len >= GT_MIN_BYTES && d_c && ((uintptr_t)d_c & 15) == 0 &&
         len <= ((1ull << 36) - 32) && aad_len < (1ull << 36) && (!aad_len || d_aad))
         return ghash_tensor_locked(c, d_aad, aad_len, d_c, len, d_out, (cudaStream_t)stream);
     int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, true, len, aad_len, &p, &blocks);

@@ -13,7 +13,7 @@ struct gcm_ctx {
     int sm_count;
     int grid;          // CTAs of the fused kernel at most (default: one per SM)
     int threads;       // threads per CTA (512 default, 256 / 384 alternatives)
-    int engine;        // GCM_GHASH_TABLE / GCM_GHASH_TENSOR: which single-message kernel multiplies by K (gcm_set_ghash_engine)
+    int engine;        // GCM_GHASH_TABLE / _TENSOR / _AUTO (gcm_set_ghash_engine)
     // device state, one slab
     uint8_t  *d_slab;
     size_t    slab_bytes;

@@ -64,6 +64,12 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ bool tc_elect()
+{
+    uint32_t pred;
+    asm volatile("{ .reg .pred p; elect.sync _|p, 0xFFFFFFFF; selp.u32 %0, 1, 0, p; }" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tc_commit(uint64_t *bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -294,12 +300,15 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
     const uint32_t tbase = *tslot;
 
     if (warp >= TC_NW) {
-        // ---- the issuing lane of group g: its slices in order -------------------------------------------------
-        if (lane == 0) {
+        // ---- the issuing warp of group g: its slices in order.  Every lane walks the loop, so that addresses and
+        // descriptors are warp-uniform and sit in uniform registers (UTCOMMA takes no others; from a single lane of a
+        // divergent branch the compiler feeds it through R2UR + election loops); one elected lane issues ----------
+        {
+            const uint32_t tb = __shfl_sync(0xFFFFFFFFu, tbase, 0);
             const uint32_t g = warp - TC_NW;
             uint64_t *full = bars + 1 + 2 * g, *empty = bars + 7 + 2 * g;
             mbar_wait(bars + 0, 0);
-            const uint32_t bm = smem_u32(sm + TC_BMAT_OFF), sf = tbase + TC_COL_SF;
+            const uint32_t bm = smem_u32(sm + TC_BMAT_OFF), sf = tb + TC_COL_SF;
             uint32_t n = 0, left = rmax;
             for (uint32_t c = 0; left; c++) {
                 const uint32_t ell = left < TC_L ? left : TC_L;
@@ -312,11 +321,14 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
                     const uint64_t b1 = tc_smem_desc(bm + e * TC_BMAT_BYTES + 4096, 2048, 128);
                     mbar_wait(full + slot, (n >> 1) & 1);
                     tc_fence_after();
-                    const uint32_t a = tbase + TC_COL_RING + 32 * g + 16 * slot;
-                    tc_mma(tbase + 128 * g, a, b0, sf, j != 0);
-                    tc_mma(tbase + 128 * g, a + 8, b1, sf, 1);
-                    tc_commit(empty + slot);
-                    if (j + 1 == nsl) tc_commit(bars + 13 + g);
+                    const uint32_t a = tb + TC_COL_RING + 32 * g + 16 * slot;
+                    if (tc_elect()) {
+                        tc_mma(tb + 128 * g, a, b0, sf, j != 0);
+                        tc_mma(tb + 128 * g, a + 8, b1, sf, 1);
+                        tc_commit(empty + slot);
+                        if (j + 1 == nsl) tc_commit(bars + 13 + g);
+                    }
+                    __syncwarp();
                 }
             }
         }

@@ -15,6 +15,7 @@ GCM_OK, GCM_ERR_AUTH, GCM_ERR_ARG, GCM_ERR_LEN, GCM_ERR_CUDA, GCM_ERR_NOMEM, GCM
 GCM_PHASE_SLOTS = 8
 GCM_GHASH_TABLE = 0
 GCM_GHASH_TENSOR = 1
+GCM_GHASH_AUTO = 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libb200gcm.so")
