@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-mib", type=float, default=384.0)
     ap.add_argument("--workload", default="c5",
-                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c2", "c3", "c4", "latency", "frame", "datasum", "phases", "sizes"],
+                    choices=["c5", "c5-decrypt", "c5-ghash", "c5-aes128", "c5-tensor", "c5-aes128-tensor", "c2", "c3", "c4", "latency", "frame", "datasum", "phases", "sizes"],
                     help="c5 = the headline (default); the others are the supplementary measurements of DESIGN.md section 10")
     return ap.parse_args()
 
@@ -189,6 +189,36 @@ def roofline_dict(pb: dict, achieved: float, peaks: dict, hbm_bytes_per_byte: in
         r["peak_measured_rates"] = pb["gbs_measured_rates"]
         r["frac_measured_rates"] = achieved / pb["gbs_measured_rates"]
     return r
+
+
+def tensor_roofline(gbs: float, sm_count: int, sm_mhz: float, peaks: dict) -> dict:
+    """Roofline of gcm_ghash_tc_kernel.  Work: one 128 x 128 bit matrix-vector product per 16-byte block = 2 x 16,384
+    flop on e2m1 (fp4) operands.  `peak` follows the contract: the measured dense bf16 rate of MEASURED_PEAKS.json
+    (cuBLAS, burst) x the nominal fp4 : bf16 ratio of 4 (9 / 2.25 PFLOP/s).  cuBLAS runs power-capped near 1.3 GHz,
+    this kernel at the full SM clock, so the fraction can exceed 1; the tight bound is the instruction rate: a
+    128 x 128 x 64 kind::mxf4 MMA takes 64 SM-cycles (measured with back-to-back MMAs on this device), i.e. one block
+    per SM-cycle."""
+    flop_per_byte = 2.0 * 128 * 128 / 16.0
+    achieved = gbs * 1e9 * flop_per_byte / 1e12
+    r = {"bound": "tensor", "unit": "TFLOP/s", "achieved": achieved, "dtype": "fp4 e2m1 (kind::mxf4), fp32 accumulate",
+         "flop_per_payload_byte": flop_per_byte, "traffic": None}
+    bf16 = peaks.get("bf16_tflops")
+    if bf16:
+        r.update(peak=4.0 * float(bf16), frac=achieved / (4.0 * float(bf16)),
+                 peak_how="bf16_tflops of MEASURED_PEAKS.json (%s) x 4 (nominal fp4 : bf16)" % peaks["_source"])
+    else:
+        r.update(peak=4.0 * 1590.0, frac=achieved / (4.0 * 1590.0), peak_how="fallback 1.59 PFLOP/s bf16 x 4 (of fallback)")
+    issue = sm_count * sm_mhz * 1e6 * 16.0 / 1e9          # GB/s at one block per SM-cycle
+    r.update(peak_mma_issue_rate_gbs=issue, frac_of_mma_issue_rate=gbs / issue,
+             hbm={"achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s", "frac": gbs / float(peaks["hbm_gbs"]),
+                  "of": peaks["_source"]})
+    return r
+
+
+def step_with(ctx, aad, ct, stream, G):
+    import torch
+    d_s = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    return lambda: G.gcm_ghash_async(ctx, aad, ct, d_s, stream)
 
 
 def traffic_per_launch(payload_bytes: int):
@@ -538,10 +568,10 @@ def run_extra(args):
     line = {"unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warm, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic", "supplementary": True}
 
-    if w in ("c5-decrypt", "c5-ghash", "c5-aes128", "c2"):
+    if w in ("c5-decrypt", "c5-ghash", "c5-aes128", "c5-tensor", "c5-aes128-tensor", "c2"):
         n = (256 << 20) if w == "c2" else int(args.size_mib * (1 << 20))
         m = workloads.config_c2(payload_bytes=0) if w == "c2" else workloads.config_c5(payload_bytes=n, with_payload=False)
-        key = m.key[:16] if w == "c5-aes128" else m.key
+        key = m.key[:16] if w.startswith("c5-aes128") else m.key
         nr = 10 if len(key) == 16 else 14
         pt = rand_bytes(n, workloads.SEEDS["C2" if w == "c2" else "C5"])
         ct = torch.empty(n, dtype=torch.uint8, device="cuda")
@@ -549,6 +579,8 @@ def run_extra(args):
         d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
         d_status = torch.zeros(1, dtype=torch.int32, device="cuda")
         ctx = G.gcm_init(key)
+        if w.endswith("-tensor"):
+            G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)     # gcm_tc.cu: the fused kernel with GHASH on the tensor cores
         G.gcm_encrypt_async(ctx, m.iv, aad, pt, ct, d_tag, stream)
         if w == "c5-decrypt":
             back = torch.empty(n, dtype=torch.uint8, device="cuda")
@@ -566,12 +598,41 @@ def run_extra(args):
             assert int(d_status.item()) == 0 and torch.equal(back[:1 << 20], pt[:1 << 20])
         G.gcm_destroy(ctx)
         gbs = steps * n / (total_ms * 1e-3) / 1e9
-        key_mix = {"c5-decrypt": "fused_aes256_dec", "c5-ghash": "fused_ghash", "c5-aes128": "fused_aes128_enc", "c2": "fused_aes256_enc"}[w]
+        key_mix = {"c5-decrypt": "fused_aes256_dec", "c5-ghash": "fused_ghash", "c5-aes128": "fused_aes128_enc", "c2": "fused_aes256_enc",
+                   "c5-tensor": "fused_aes256_enc", "c5-aes128-tensor": "fused_aes128_enc"}[w]
         pb = pipe_bound_gbs(key_mix, nr, sm_count, sm_mhz, G.gcm_measure_pipe_rates(), ghash_only=(mode == "ghash"))
+        if w == "c5-ghash":
+            # The default engine (GCM_GHASH_AUTO) ran: for a long aligned input that is gcm_ghash_tc_kernel, GHASH as a
+            # GF(2) matrix product on tcgen05.mma kind::mxf4, between two short row-kernel launches (AAD; tail + length
+            # block).  Its bound is the tensor pipe; the table kernel is timed beside it against its own bound.
+            ctx = G.gcm_init(key)
+            G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TABLE)
+            tab_ms, _, _ = timed(step_with(ctx, aad, ct, stream, G))
+            G.gcm_destroy(ctx)
+            tab_gbs = steps * n / (tab_ms * 1e-3) / 1e9
+            table = roofline_dict(pb, tab_gbs, peaks, 1)
+            line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
+                        config={"workload": "%s: %s, %d-byte message, 2880-byte AAD; default engine (tensor cores)" % (w, what, n),
+                                "payload_bytes": n},
+                        gpu_launches=3 * steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks),
+                        table_engine={"value": tab_gbs, "unit": UNIT, "ms_per_step": tab_ms / steps, "roofline": table},
+                        ms_per_step_median=statistics.median(per))
+            print(json.dumps(line))
+            return
+        roof = roofline_dict(pb, gbs, peaks, 1 if mode == "ghash" else 2)
+        if w.endswith("-tensor"):
+            # GHASH has left the shared-memory pipe: what binds is the AES table reads alone (the second yardstick);
+            # the tcgen05.st / tcgen05.ld traffic of the tensor path adds to it and is not counted here
+            y = pb["yardsticks"]
+            what += ", GHASH on the tensor cores (gcm_tc.cu)"
+            roof.update(peak=y["aes_reads_only_gbs"], frac=gbs / y["aes_reads_only_gbs"],
+                        pipe="shared-memory data pipe (LSU): %.1f bank-lanes per block for the AES table reads alone; the multiply "
+                             "by K runs on tcgen05.mma kind::mxf4" % y["aes_reads_only_lanes"])
+            for k in ("frac_with_global_wavefronts", "counts_per_block", "peak_measured_rates", "frac_measured_rates"):
+                roof.pop(k, None)
         line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
                     config={"workload": "%s: %s, %d-byte message, 2880-byte AAD" % (w, what, n), "payload_bytes": n},
-                    gpu_launches=launches * steps, clocks=clocks,
-                    roofline=roofline_dict(pb, gbs, peaks, 1 if mode == "ghash" else 2),
+                    gpu_launches=launches * steps, clocks=clocks, roofline=roof,
                     ms_per_step_median=statistics.median(per))
     elif w == "c3":
         msgs = workloads.config_c3()
