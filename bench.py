@@ -202,6 +202,11 @@ def tensor_roofline(gbs: float, sm_count: int, sm_mhz: float, peaks: dict) -> di
     achieved = gbs * 1e9 * flop_per_byte / 1e12
     r = {"bound": "tensor", "unit": "TFLOP/s", "achieved": achieved, "dtype": "fp4 e2m1 (kind::mxf4), fp32 accumulate",
          "flop_per_payload_byte": flop_per_byte, "traffic": None}
+    try:            # dram bytes of one launch from the committed ncu --set full capture, scaled by size
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))["ghash_tc"]
+        r["traffic_per_payload_byte"] = t["dram_bytes_per_payload_byte"]
+    except Exception:
+        pass
     bf16 = peaks.get("bf16_tflops")
     if bf16:
         r.update(peak=4.0 * float(bf16), frac=achieved / (4.0 * float(bf16)),
@@ -617,6 +622,9 @@ def run_extra(args):
                         gpu_launches=3 * steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks),
                         table_engine={"value": tab_gbs, "unit": UNIT, "ms_per_step": tab_ms / steps, "roofline": table},
                         ms_per_step_median=statistics.median(per))
+            tpb = line["roofline"].pop("traffic_per_payload_byte", None)
+            if tpb is not None:
+                line["roofline"]["traffic"] = tpb * n
             print(json.dumps(line))
             return
         roof = roofline_dict(pb, gbs, peaks, 1 if mode == "ghash" else 2)

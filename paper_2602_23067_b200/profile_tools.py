@@ -35,7 +35,8 @@ RAW_METRICS = (
     r"l1tex__data_pipe_lsu_wavefronts_mem_shared.sum$|l1tex__data_pipe_lsu_wavefronts_mem_shared_op_(ld|st).sum$|"
     r"l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum$|lts__t_bytes.sum$|"
     r"stalled_(short_scoreboard|mio_throttle|long_scoreboard|math_pipe_throttle|not_selected|wait|barrier)_per_issue_active.ratio|"
-    r"sm__warps_active.avg.pct")
+    r"sm__warps_active.avg.pct|sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_(elapsed|active)$|"
+    r"sm__inst_executed_pipe_tensor|smsp__inst_executed_pipe_(uniform|tmem)")
 
 ALU = {"LOP3", "PRMT", "SHF", "IADD3", "IADD", "ISETP", "SEL", "LEA", "VIADD", "PLOP3", "MOV", "IABS", "IMNMX", "VIMNMX",
        "POPC", "FLO", "BREV", "SGXT", "BMSK", "LOP", "R2P", "P2R", "CS2R", "I2FP", "FSETP", "FMNMX", "VABSDIFF"}
