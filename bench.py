@@ -191,7 +191,7 @@ def roofline_dict(pb: dict, achieved: float, peaks: dict, hbm_bytes_per_byte: in
     return r
 
 
-def tensor_roofline(gbs: float, sm_count: int, sm_mhz: float, peaks: dict) -> dict:
+def tensor_roofline(gbs: float, sm_count: int, sm_mhz: float, peaks: dict, rates: dict = None) -> dict:
     """Roofline of gcm_ghash_tc_kernel.  Work: one 128 x 128 bit matrix-vector product per 16-byte block = 2 x 16,384
     flop on e2m1 (fp4) operands.  `peak` follows the contract: the measured dense bf16 rate of MEASURED_PEAKS.json
     (cuBLAS, burst) x the nominal fp4 : bf16 ratio of 4 (9 / 2.25 PFLOP/s).  cuBLAS runs power-capped near 1.3 GHz,
@@ -213,8 +213,9 @@ def tensor_roofline(gbs: float, sm_count: int, sm_mhz: float, peaks: dict) -> di
                  peak_how="bf16_tflops of MEASURED_PEAKS.json (%s) x 4 (nominal fp4 : bf16)" % peaks["_source"])
     else:
         r.update(peak=4.0 * 1590.0, frac=achieved / (4.0 * 1590.0), peak_how="fallback 1.59 PFLOP/s bf16 x 4 (of fallback)")
-    issue = sm_count * sm_mhz * 1e6 * 16.0 / 1e9          # GB/s at one block per SM-cycle
-    r.update(peak_mma_issue_rate_gbs=issue, frac_of_mma_issue_rate=gbs / issue,
+    blocks_per_cycle = float(rates["mma_mxf4_blocks"]) if rates and rates.get("mma_mxf4_blocks") else 1.0
+    issue = sm_count * sm_mhz * 1e6 * 16.0 * blocks_per_cycle / 1e9      # GB/s at the measured MMA rate (nominal: one block per SM-cycle)
+    r.update(mma_blocks_per_sm_cycle=blocks_per_cycle, peak_mma_issue_rate_gbs=issue, frac_of_mma_issue_rate=gbs / issue,
              hbm={"achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s", "frac": gbs / float(peaks["hbm_gbs"]),
                   "of": peaks["_source"]})
     return r
@@ -619,7 +620,7 @@ def run_extra(args):
             line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
                         config={"workload": "%s: %s, %d-byte message, 2880-byte AAD; default engine (tensor cores)" % (w, what, n),
                                 "payload_bytes": n},
-                        gpu_launches=3 * steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks),
+                        gpu_launches=3 * steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks, G.gcm_measure_pipe_rates()),
                         table_engine={"value": tab_gbs, "unit": UNIT, "ms_per_step": tab_ms / steps, "roofline": table},
                         ms_per_step_median=statistics.median(per))
             tpb = line["roofline"].pop("traffic_per_payload_byte", None)

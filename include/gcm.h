@@ -130,6 +130,8 @@ enum {
     GCM_RATE_IMAD,          /* 32-bit integer multiply-add                                           */
     GCM_RATE_IMAD_WIDE,     /* 32 x 32 + 64 -> 64 multiply-add (the generic GF(2^128) product)       */
     GCM_RATE_LOP3_IMAD,     /* LOP3 and IMAD interleaved 1:1 (both pipes), operations of both kinds  */
+    GCM_RATE_MMA_MXF4,      /* tensor pipe: 128 x 128 x 64 tcgen05.mma kind::mxf4 back to back, in GHASH blocks
+                               (128 x 128 bit products) per SM-cycle, not thread-operations                 */
     GCM_RATE_COUNT
 };
 GCM_API int gcm_measure_pipe_rates(double *rates, int n);

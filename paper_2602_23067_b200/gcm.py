@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = [
     "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_debug_row_layout", "gcm_debug_plan_chunks",
     "gcm_measure_pipe_rates",
 ]
-RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad"]
+RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad", "mma_mxf4_blocks"]
 
 
 class GcmError(RuntimeError):
