@@ -494,7 +494,7 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     GcmParams p;
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
-    if (c->engine != GCM_GHASH_TABLE && len >= GT_MIN_BYTES && d_c && ((uintptr_t)d_c & 15) == 0 &&
+    if (c->engine != GCM_GHASH_TABLE && len >= (c->engine == GCM_GHASH_TENSOR ? GT_MIN_BYTES : GT_AUTO_BYTES) && d_c && ((uintptr_t)d_c & 15) == 0 &&
         len <= ((1ull << 36) - 32) && aad_len < (1ull << 36) && (!aad_len || d_aad))
         return ghash_tensor_locked(c, d_aad, aad_len, d_c, len, d_out, (cudaStream_t)stream);
     int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, true, len, aad_len, &p, &blocks);

@@ -145,7 +145,7 @@ def test_tensor_engine_equals_table_engine_at_64_mib(G, oracle):
 
 @pytest.mark.parametrize("engine", ["auto", "tensor"])
 def test_ghash_stretch_kernel_shapes(G, oracle, engine):
-    """gcm_ghash_async over at least 4 MiB of aligned input: gcm_ghash_tc_kernel takes the whole 32 KiB chunks, the row
+    """gcm_ghash_async over at least 4 MiB (engine TENSOR) / 96 MiB (default engine) of aligned input: gcm_ghash_tc_kernel takes the whole 32 KiB chunks, the row
     kernel the AAD in front and the ragged rest and the length block behind (three chained launches).  Lengths on
     and around the threshold and the chunk size, AAD 0 / 1 / 16 / 2880 bytes, grids of 1, 5, 148 and 300 CTAs (more
     CTAs than chunks included), both key sizes; one unaligned and one short input, which must take the row kernel."""
@@ -154,6 +154,8 @@ def test_ghash_stretch_kernel_shapes(G, oracle, engine):
     M = 4 << 20
     cases = [(M, 0, 0), (M + 1, 16, 0), (M - 1, 2880, 0), (M + 32768, 1, 5), (M + 32767, 0, 1), (M + 32769, 17, 148),
              (5 * M + 12345, 2880, 300), (148 * 32768 * 2, 0, 0), (148 * 32768 * 2 + 32768 * 3 + 15, 100, 0), (3 * M, 16, 1)]
+    if engine == "auto":        # the default engine takes the tensor path from 96 MiB on; below that the table kernel
+        cases = [(24 * M, 0, 0), (24 * M - 1, 16, 0), (24 * M + 32769, 2880, 0), (25 * M + 7, 1, 40)]
     for klen in (16, 32):
         key = rnd(rng, klen).tobytes()
         h = oracle.hash_subkey(key)
