@@ -608,9 +608,8 @@ def run_extra(args):
                    "c5-tensor": "fused_aes256_enc", "c5-aes128-tensor": "fused_aes128_enc"}[w]
         pb = pipe_bound_gbs(key_mix, nr, sm_count, sm_mhz, G.gcm_measure_pipe_rates(), ghash_only=(mode == "ghash"))
         if w == "c5-ghash":
-            # The default engine (GCM_GHASH_AUTO) ran: for a long aligned input that is gcm_ghash_tc_kernel, GHASH as a
-            # GF(2) matrix product on tcgen05.mma kind::mxf4, between two short row-kernel launches (AAD; tail + length
-            # block).  Its bound is the tensor pipe; the table kernel is timed beside it against its own bound.
+            # The default engine (GCM_GHASH_AUTO) ran: for a long aligned input that is ONE launch of gcm_ghash_tc_kernel,
+            # GHASH as a GF(2) matrix product on tcgen05.mma kind::mxf4 over [pad | AAD | C | length block].  Its bound is the tensor pipe; the table kernel is timed beside it against its own bound.
             ctx = G.gcm_init(key)
             G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TABLE)
             tab_ms, _, _ = timed(step_with(ctx, aad, ct, stream, G))
@@ -620,7 +619,7 @@ def run_extra(args):
             line.update(metric="%s GB/s (device-timed, %d MiB msg)" % (what, n >> 20), value=gbs, ms_per_step=total_ms / steps,
                         config={"workload": "%s: %s, %d-byte message, 2880-byte AAD; default engine (tensor cores)" % (w, what, n),
                                 "payload_bytes": n},
-                        gpu_launches=3 * steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks, G.gcm_measure_pipe_rates()),
+                        gpu_launches=steps, clocks=clocks, roofline=tensor_roofline(gbs, sm_count, sm_mhz, peaks, G.gcm_measure_pipe_rates()),
                         table_engine={"value": tab_gbs, "unit": UNIT, "ms_per_step": tab_ms / steps, "roofline": table},
                         ms_per_step_median=statistics.median(per))
             tpb = line["roofline"].pop("traffic_per_payload_byte", None)

@@ -105,10 +105,10 @@ GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
  *                     0 / 1 operands, accumulators in TMEM, parity of the counts.  The single-message encrypt / decrypt /
  *                     GHASH calls run gcm_tc.cu (CTAs of 12 warps that take rows + 3 that issue the MMAs; `threads` of
  *                     gcm_set_geometry is ignored, `grid` kept), and gcm_ghash_async on at least 4 MiB of 16-byte
- *                     aligned input runs gcm_ghash_tc.cu over the whole 32 KiB chunks of it;
+ *                     aligned input runs gcm_ghash_tc.cu (one launch over pad | AAD | C | length block);
  *   GCM_GHASH_AUTO    (default) what is fastest on a B200: the table for encrypt / decrypt, the tensor cores for
- *                     gcm_ghash_async on at least 96 MiB of aligned input (below that the one launch of the table
- *                     kernel beats the three chained launches of the tensor path).
+ *                     gcm_ghash_async on at least 32 MiB of aligned input (below that the table kernel's shorter
+ *                     prologue wins).
  * Results are bit-identical under all three.  The batched calls and the latency kernel are not affected.
  * Returns GCM_OK / GCM_ERR_ARG.
  */

@@ -171,7 +171,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     size_t o_hpow = take((GCM_STRIDE + 1) * 16), o_hx = take(HX_ENTRIES * 16);
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
     size_t o_cnt = take(4), o_tag = take(16), o_status = take(4), o_bmat = take(TC_BMAT_TOTAL);
-    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES), o_gt = take(64);
+    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES);
     c->slab_bytes = off;
     cudaError_t e = cudaSuccess;
     {
@@ -198,7 +198,6 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     c->d_bmat = (uint4 *)(c->d_slab + o_bmat);
     c->d_bmat2 = (uint4 *)(c->d_slab + o_bmat2);
     c->d_ktab2 = (uint4 *)(c->d_slab + o_ktab2);
-    c->d_gt = (uint4 *)(c->d_slab + o_gt);
 
     int rc = GCM_OK;
     do {
@@ -451,39 +450,16 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
     return GCM_OK;
 }
 
-// GHASH only, tensor engine, long aligned input: three links of a chunk chain on the caller's stream.
-//   1. the AAD (if any) through the row kernel            -> state d_gt[0]
-//   2. the first nchunks * 32 KiB of C on the tensor cores -> state d_gt[1], and H^(blocks of link 3) -> d_gt[2]
-//   3. the rest of C and the length block through the row kernel, chained behind d_gt[1]
+// GHASH only on the tensor cores: one launch of gcm_ghash_tc_kernel over [pad | AAD | C | length block].
 static int ghash_tensor_locked(gcm_ctx *c, const void *d_aad, uint64_t aad_len, const void *d_c, uint64_t len,
                                void *d_out, cudaStream_t s)
 {
-    const uint64_t nchunks = len / (16ull * GT_CHUNK_BLOCKS), bulk = nchunks * 16ull * GT_CHUNK_BLOCKS;
-    GcmParams p;
-    int blocks = 0, rc;
-    cudaError_t e;
-    if (aad_len) {
-        rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, nullptr, 0, nullptr, 0, false, len, aad_len, &p, &blocks);
-        if (rc != GCM_OK) return rc;
-        p.chain_out = c->d_gt + 0;
-        e = gcm_launch_fused(c, MODE_GHASH, blocks, p, s);
-        secure_zero(&p, sizeof(p));
-        if (e != cudaSuccess) return gcm_cuda_fail(e);
-    }
-    const uint64_t tail = len - bulk;
-    blocks = (int)(nchunks < (uint64_t)c->grid ? nchunks : (uint64_t)c->grid);
+    const uint64_t nchunks = ghash_tc_chunks(aad_len, len);
+    const int blocks = (int)(nchunks < (uint64_t)c->grid ? nchunks : (uint64_t)c->grid);
     c->ticket_next += (unsigned)blocks;
-    e = launch_ghash_tc(blocks, (const uint8_t *)d_c, nchunks, c->d_bmat2, c->d_ktab2, c->d_hx, c->d_partials, c->d_counter,
-                        c->ticket_next - 1, aad_len ? c->d_gt + 0 : nullptr, c->d_gt + 1, (tail + 15) / 16 + 1, c->d_gt + 2, s);
+    cudaError_t e = launch_ghash_tc(blocks, (const uint8_t *)d_aad, aad_len, (const uint8_t *)d_c, len, c->d_bmat2, c->d_ktab2, c->d_hx,
+                                    c->d_partials, c->d_counter, c->ticket_next - 1, (uint4 *)d_out, s);
     if (e != cudaSuccess) { c->ticket_next -= (unsigned)blocks; return gcm_cuda_fail(e); }
-    rc = gcm_build_params(c, MODE_GHASH, nullptr, nullptr, 0, (const uint8_t *)d_c + bulk, tail, nullptr, 0, true, len, aad_len, &p, &blocks);
-    if (rc != GCM_OK) return rc;
-    p.chain_in = c->d_gt + 1;
-    p.chain_pow = c->d_gt + 2;
-    p.tag_out = (uint4 *)d_out;
-    e = gcm_launch_fused(c, MODE_GHASH, blocks, p, s);
-    secure_zero(&p, sizeof(p));
-    if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;
 }
 
@@ -495,7 +471,7 @@ extern "C" int gcm_ghash_async(gcm_ctx *c, const void *d_aad, uint64_t aad_len, 
     int blocks = 0;
     if (!d_out) return GCM_ERR_ARG;
     if (c->engine != GCM_GHASH_TABLE && len >= (c->engine == GCM_GHASH_TENSOR ? GT_MIN_BYTES : GT_AUTO_BYTES) && d_c && ((uintptr_t)d_c & 15) == 0 &&
-        len <= ((1ull << 36) - 32) && aad_len < (1ull << 36) && (!aad_len || d_aad))
+        len <= ((1ull << 36) - 32) && aad_len < (1ull << 32) && (!aad_len || d_aad))
         return ghash_tensor_locked(c, d_aad, aad_len, d_c, len, d_out, (cudaStream_t)stream);
     int rc = gcm_build_params(c, MODE_GHASH, nullptr, d_aad, aad_len, d_c, len, nullptr, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;

@@ -42,8 +42,8 @@
 #define GT_CHUNK_BLOCKS   (128 * GT_L)
 #define GT_BMAT_TOTAL     (GT_L * TC_BMAT_BYTES)
 #define GT_MIN_BYTES      (4ull << 20)   /* GCM_GHASH_TENSOR: shorter messages stay with the row kernels */
-#define GT_AUTO_BYTES     (96ull << 20)  /* GCM_GHASH_AUTO: the three chained launches cost about 13 us more than the one
-                                            launch of the table kernel and win from about 100 MiB on (measured) */
+#define GT_AUTO_BYTES     (32ull << 20)  /* GCM_GHASH_AUTO: its prologue (192 KB of tables, TMEM) costs the tensor kernel about 3 us
+                                            more than the table kernel; it is level at 32 MiB and ahead beyond */
 
 #define GCM_MAX_THREADS 512
 #define GCM_MAX_GRID    4096

@@ -6,7 +6,7 @@
 // fp32 -- but laid out for a kernel that has nothing else to do:
 //
 //   * ONE tile per CTA.  The CTA's run of blocks is cut into slices of 128 consecutive blocks; block 128 t + j of the
-//     run is row j (TMEM lane j) of slice t.  Twelve producer warps load (LDG.128, four loads in flight per lane),
+//     run is row j (TMEM lane j) of slice t.  A load warp brings the slices into shared memory (one bulk copy of 2 KB each, 16 in flight); twelve producer warps take their 16 bytes,
 //     expand the bits to nibbles (five ALU instructions per word) and store their 32 rows of a slice straight into
 //     TMEM (tcgen05.st); slice t belongs to the four warps with (warp >> 2) == t % 3, one per lane quarter.
 //   * A chunk is 16 slices: row j of the accumulator becomes  Z_j = sum_t X_(128 t + j) . K^(15 - t),  K = H^128, by
@@ -18,8 +18,9 @@
 //     kernel (ghash_mul_k, table of H^2048): one table multiply per 16 blocks instead of one per block.
 //   * End of the run: Y_j . H^(128 - j), XOR over the rows, times H^(blocks of the stretch behind the run), partial
 //     to global memory, last-CTA-done as in gcm_fused.cu; the finisher adds the state handed in (chain_in . H^N) and
-//     hands the new state on (chain_out): the stretch is one link of the chunk chain of GcmParams, with the fused
-//     kernel doing the AAD in front and the ragged tail and length block behind (gcm_api.cu: gcm_ghash_async).
+//     writes GHASH_H(A, C).  The kernel covers the WHOLE virtual sequence [pad | AAD | C | length block] (pad = leading
+//     zero blocks up to a whole number of chunks): the few slices at both ends that are not whole blocks of C are put
+//     together by the load warp with ordinary loads, all others arrive by bulk copy.  One launch per call.
 //
 // Bound: 32 MMAs of 64 cycles per 2048 blocks = one block per SM-cycle on the tensor pipe (4.65 TB/s at 1965 MHz),
 // against two cycles per block on the shared-memory pipe for the table multiply and 0.73 for HBM (1 B/B at 6.5 TB/s).
@@ -31,6 +32,7 @@
 #include "gcm_device.cuh"
 
 #include <atomic>
+#include <string.h>
 
 #define GT_PRODUCERS  12                             /* 17 warps are allotted registers as 20: 96 per thread */
 #define GT_THREADS    (32 * (GT_PRODUCERS + 4 + 2))     /* + 4 read-back warps, the MMA warp, the load warp */
@@ -49,8 +51,14 @@ static_assert(GT_STAGES % (GT_PRODUCERS / 4) != 0 || true, "");
 static_assert(GT_RING % 4 == 0 && GT_L % 4 == 0, "the issue loop takes four slices per trip");
 static_assert(GT_BMAT_TOTAL == KTAB_OFF, "the matrices fill the 128 KB in front of the multiplier table");
 
+// The kernel hashes the virtual block sequence  [pad zero blocks | AAD blocks | C blocks | length block]  of
+// nchunks * GT_CHUNK_BLOCKS blocks: pad (leading zero blocks are free in GHASH) rounds it up to whole chunks, so the
+// length block is the last block of the last chunk and nothing is left for another launch.
 struct GhashTcParams {
-    const uint8_t *in;          // 16-byte aligned; nchunks * GT_CHUNK_BLOCKS * 16 bytes
+    const uint8_t *in;          // C, 16-byte aligned
+    const uint8_t *aad;
+    uint64_t len, aad_len;      // bytes
+    uint64_t pad, base;         // leading zero blocks; virtual index of C block 0 = pad + AAD blocks
     uint64_t nchunks;
     const uint4 *bmat2;         // GT_BMAT_TOTAL
     const uint4 *ktab2;         // KTAB_BYTES: Shoup table of H^(128 * GT_L)
@@ -236,20 +244,66 @@ gcm_ghash_tc_kernel(const __grid_constant__ GhashTcParams p)
     } else if (warp == GT_PRODUCERS + 5) {
         // ---- the load warp: one bulk copy (TMA 1-D) per slice of 2 KB, GT_STAGES of them in flight.  Every lane walks the
         // loop (addresses stay warp-uniform: UBLKCP takes uniform registers), one elected lane issues -----------------
-        const uint8_t *src = p.in + 16 * (c0 * GT_CHUNK_BLOCKS);
         const uint32_t st0 = smem_u32(sm + GT_STAGE_OFF), sf0 = smem_u32(sfull), se0 = smem_u32(sempty);
+        const uint64_t n_full = p.len / 16, n_cb = (p.len + 15) / 16, last = p.nchunks * GT_CHUNK_BLOCKS - 1;
+        const uint64_t v_run = c0 * GT_CHUNK_BLOCKS;                   // virtual index of the run's first block
+        // slices [t_lo, t_hi) of the run hold whole blocks of C only and arrive by bulk copy; the (at most three) others,
+        // at either end of the message, are put together by hand
+        uint32_t t_lo = 0, t_hi = 0;
+        {
+            const uint64_t lo = p.base > v_run ? (p.base - v_run + 127) / 128 : 0;
+            const uint64_t end = p.base + n_full;                       // first virtual block that is not a whole block of C
+            const uint64_t hi = end > v_run ? (end - v_run) / 128 : 0;
+            t_lo = (uint32_t)(lo < T ? lo : T);
+            t_hi = (uint32_t)(hi < T ? hi : T);
+            if (t_hi < t_lo) t_hi = t_lo;
+        }
         pdl_wait();
         uint32_t stage = 0, sph = 1, sa = st0, fa = sf0, ea = se0;
+        const uint8_t *src = p.in + 16 * (v_run + 128ull * t_lo - p.base);      // used from slice t_lo on
+        uint32_t tt = 0;
+        while (tt < T) {
+            if (tt >= t_lo && tt < t_hi) {
 #pragma unroll 1
-        for (uint32_t tt = 0; tt < T; tt++) {
+                for (; tt < t_hi; tt++) {                               // the steady state: nothing but additions
+                    mbar_wait_addr(ea, sph);
+                    if (gt_elect()) {
+                        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], 2048;" ::"r"(fa) : "memory");
+                        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 2048, [%2];"
+                                     ::"r"(sa), "l"(src), "r"(fa) : "memory");
+                    }
+                    __syncwarp();
+                    src += 2048; sa += 2048; fa += 8; ea += 8;
+                    if (++stage == GT_STAGES) { stage = 0; sph ^= 1; sa = st0; fa = sf0; ea = se0; }
+                }
+                continue;
+            }
             mbar_wait_addr(ea, sph);
-            if (gt_elect()) {
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], 2048;" ::"r"(fa) : "memory");
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 2048, [%2];"
-                             ::"r"(sa), "l"(src), "r"(fa) : "memory");
+            const uint64_t v0 = v_run + 128ull * tt;
+#pragma unroll 1
+            for (uint32_t k = 0; k < 4; k++) {
+                const uint64_t v = v0 + 32 * k + lane;
+                uint4 x = make_uint4(0, 0, 0, 0);
+                if (v == last) {                                        // a10: BE64(8 a) || BE64(8 len)
+                    const uint64_t abits = p.aad_len * 8, cbits = p.len * 8;
+                    x = make_uint4(bswap32((uint32_t)(abits >> 32)), bswap32((uint32_t)abits), bswap32((uint32_t)(cbits >> 32)), bswap32((uint32_t)cbits));
+                } else if (v >= p.base) {
+                    const uint64_t g = v - p.base;
+                    if (g < n_cb) {
+                        const uint64_t rem = p.len - 16 * g;
+                        x = rem >= 16 ? __ldg(reinterpret_cast<const uint4 *>(p.in + 16 * g)) : load_bytes(p.in + 16 * g, (uint32_t)rem);
+                    }
+                } else if (v >= p.pad) {
+                    const uint64_t u = v - p.pad, rem = p.aad_len - 16 * u;
+                    x = load_bytes(p.aad + 16 * u, rem < 16 ? (uint32_t)rem : 16u);
+                }
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(sa + 16 * (32 * k + lane)), "r"(x.x), "r"(x.y), "r"(x.z), "r"(x.w) : "memory");
             }
             __syncwarp();
-            src += 2048; sa += 2048; fa += 8; ea += 8;
+            if (gt_elect()) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(fa) : "memory");
+            __syncwarp();
+            tt++;
+            sa += 2048; fa += 8; ea += 8;
             if (++stage == GT_STAGES) { stage = 0; sph ^= 1; sa = st0; fa = sf0; ea = se0; }
         }
     } else if (warp == GT_PRODUCERS + 4) {
@@ -338,7 +392,7 @@ gcm_ghash_tc_kernel(const __grid_constant__ GhashTcParams p)
     if (lane == 0) {
         if (p.chain_in != nullptr) tot = xor4(tot, gf_mul_mem(*p.chain_in, gt_pow(p.hx, p.nchunks * GT_CHUNK_BLOCKS)));
         *p.chain_out = tot;
-        *p.pow_out = gt_pow(p.hx, p.exp_next);
+        if (p.pow_out != nullptr) *p.pow_out = gt_pow(p.hx, p.exp_next);
     }
 }
 
@@ -394,18 +448,24 @@ void launch_ghash_tc_setup(const uint4 *hx, uint4 *bmat2, uint4 *ktab2, cudaStre
     gcm_ghash_tc_setup_kernel<<<GT_L + 1, 128, 0, s>>>(hx, bmat2, ktab2);
 }
 
-cudaError_t launch_ghash_tc(int blocks, const uint8_t *in, uint64_t nchunks, const uint4 *bmat2, const uint4 *ktab2, const uint4 *hx,
-                            uint4 *partials, unsigned *counter, unsigned ticket_last, const uint4 *chain_in, uint4 *chain_out,
-                            uint64_t exp_next, uint4 *pow_out, cudaStream_t s)
+cudaError_t launch_ghash_tc(int blocks, const uint8_t *aad, uint64_t aad_len, const uint8_t *in, uint64_t len, const uint4 *bmat2,
+                            const uint4 *ktab2, const uint4 *hx, uint4 *partials, unsigned *counter, unsigned ticket_last, uint4 *out,
+                            cudaStream_t s)
 {
     static std::atomic<bool> configured[GCM_MAX_DEVICES];
     const void *kern = (const void *)gcm_ghash_tc_kernel;
     cudaError_t e = ensure_smem_attr(kern, configured, GT_SMEM_BYTES);
     if (e != cudaSuccess) return e;
     GhashTcParams p;
-    p.in = in; p.nchunks = nchunks; p.bmat2 = bmat2; p.ktab2 = ktab2; p.hx = hx;
+    memset(&p, 0, sizeof(p));
+    const uint64_t n_aad = (aad_len + 15) / 16, blocks_real = n_aad + (len + 15) / 16 + 1;
+    p.nchunks = ghash_tc_chunks(aad_len, len);
+    p.pad = p.nchunks * GT_CHUNK_BLOCKS - blocks_real;
+    p.base = p.pad + n_aad;
+    p.in = in; p.aad = aad; p.len = len; p.aad_len = aad_len;
+    p.bmat2 = bmat2; p.ktab2 = ktab2; p.hx = hx;
     p.partials = partials; p.counter = counter; p.ticket_last = ticket_last;
-    p.chain_in = chain_in; p.chain_out = chain_out; p.exp_next = exp_next; p.pow_out = pow_out;
+    p.chain_out = out;
     void *args[] = {(void *)&p};
     return launch_with_pdl(kern, dim3(blocks), dim3(GT_THREADS), GT_SMEM_BYTES, s, args);
 }

@@ -8,9 +8,13 @@ cudaError_t launch_tc(int nr, int mode, int blocks, const GcmParams &p, cudaStre
 // bmat[e] = bit matrix of "multiply by H^(32 e)", e = 0 .. TC_L, from the context's power table hx (once per key)
 void launch_tc_setup(const uint4 *hx, uint4 *bmat, cudaStream_t s);
 
-// gcm_ghash_tc.cu: GHASH of nchunks * GT_CHUNK_BLOCKS aligned blocks as one link of a chunk chain (chain_in may be
-// NULL); also stores H^exp_next to pow_out for the launch that follows.  Tables: launch_ghash_tc_setup, once per key.
+// gcm_ghash_tc.cu: GHASH_H(A, C) of a 16-byte-aligned C in ONE launch on the tensor cores: the virtual sequence
+// [pad | AAD | C | length block] in whole chunks of GT_CHUNK_BLOCKS.  Tables: launch_ghash_tc_setup, once per key.
+static inline uint64_t ghash_tc_chunks(uint64_t aad_len, uint64_t len)
+{
+    return ((aad_len + 15) / 16 + (len + 15) / 16 + 1 + GT_CHUNK_BLOCKS - 1) / GT_CHUNK_BLOCKS;
+}
 void launch_ghash_tc_setup(const uint4 *hx, uint4 *bmat2, uint4 *ktab2, cudaStream_t s);
-cudaError_t launch_ghash_tc(int blocks, const uint8_t *in, uint64_t nchunks, const uint4 *bmat2, const uint4 *ktab2, const uint4 *hx,
-                            uint4 *partials, unsigned *counter, unsigned ticket_last, const uint4 *chain_in, uint4 *chain_out,
-                            uint64_t exp_next, uint4 *pow_out, cudaStream_t s);
+cudaError_t launch_ghash_tc(int blocks, const uint8_t *aad, uint64_t aad_len, const uint8_t *in, uint64_t len, const uint4 *bmat2,
+                            const uint4 *ktab2, const uint4 *hx, uint4 *partials, unsigned *counter, unsigned ticket_last, uint4 *out,
+                            cudaStream_t s);

@@ -145,17 +145,19 @@ def test_tensor_engine_equals_table_engine_at_64_mib(G, oracle):
 
 @pytest.mark.parametrize("engine", ["auto", "tensor"])
 def test_ghash_stretch_kernel_shapes(G, oracle, engine):
-    """gcm_ghash_async over at least 4 MiB (engine TENSOR) / 96 MiB (default engine) of aligned input: gcm_ghash_tc_kernel takes the whole 32 KiB chunks, the row
-    kernel the AAD in front and the ragged rest and the length block behind (three chained launches).  Lengths on
-    and around the threshold and the chunk size, AAD 0 / 1 / 16 / 2880 bytes, grids of 1, 5, 148 and 300 CTAs (more
-    CTAs than chunks included), both key sizes; one unaligned and one short input, which must take the row kernel."""
+    """gcm_ghash_async over at least 4 MiB (engine TENSOR) / 32 MiB (default engine) of aligned input: one launch of
+    gcm_ghash_tc_kernel over [pad | AAD | C | length block] in whole 32 KiB chunks; the slices at both ends (pad, AAD, the
+    first blocks of C; the ragged last block, the length block) are put together by hand, the rest by bulk copy.
+    Lengths on and around the threshold and the chunk size, AAD 0 / 1 / 16 / 17 / 100 / 2880 bytes (AAD within one
+    slice and across two), grids of 1, 5, 40, 148 and 300 CTAs (more CTAs than chunks included), both key sizes; one
+    unaligned input, which must take the row kernel."""
     import workloads
     rng = np.random.default_rng(9980)
     M = 4 << 20
     cases = [(M, 0, 0), (M + 1, 16, 0), (M - 1, 2880, 0), (M + 32768, 1, 5), (M + 32767, 0, 1), (M + 32769, 17, 148),
              (5 * M + 12345, 2880, 300), (148 * 32768 * 2, 0, 0), (148 * 32768 * 2 + 32768 * 3 + 15, 100, 0), (3 * M, 16, 1)]
-    if engine == "auto":        # the default engine takes the tensor path from 96 MiB on; below that the table kernel
-        cases = [(24 * M, 0, 0), (24 * M - 1, 16, 0), (24 * M + 32769, 2880, 0), (25 * M + 7, 1, 40)]
+    if engine == "auto":        # the default engine takes the tensor path from 32 MiB on; below that the table kernel
+        cases = [(8 * M, 0, 0), (8 * M - 1, 16, 0), (8 * M + 32769, 2880, 0), (25 * M + 7, 1, 40)]
     for klen in (16, 32):
         key = rnd(rng, klen).tobytes()
         h = oracle.hash_subkey(key)
