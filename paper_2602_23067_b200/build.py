@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libb200gcm.so")
-SOURCES = ["gcm_api.cu", "gcm_setup.cu", "gcm_fused.cu", "gcm_tc.cu", "gcm_ghash_tc.cu", "gcm_small.cu", "gcm_batch.cu", "gcm_multi.cu", "gcm_host.cu", "gcm_rates.cu",
+SOURCES = ["gcm_api.cu", "gcm_setup.cu", "gcm_fused.cu", "gcm_tc.cu", "gcm_ghash_tc.cu", "gcm_tc2.cu", "gcm_small.cu", "gcm_batch.cu", "gcm_multi.cu", "gcm_host.cu", "gcm_rates.cu",
            "fits_sum.cu", "gfc_frame.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -171,7 +171,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     size_t o_hpow = take((GCM_STRIDE + 1) * 16), o_hx = take(HX_ENTRIES * 16);
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
     size_t o_cnt = take(4), o_tag = take(16), o_status = take(4), o_bmat = take(TC_BMAT_TOTAL);
-    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES);
+    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES), o_gt = take(64);
     c->slab_bytes = off;
     cudaError_t e = cudaSuccess;
     {
@@ -198,6 +198,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     c->d_bmat = (uint4 *)(c->d_slab + o_bmat);
     c->d_bmat2 = (uint4 *)(c->d_slab + o_bmat2);
     c->d_ktab2 = (uint4 *)(c->d_slab + o_ktab2);
+    c->d_gt = (uint4 *)(c->d_slab + o_gt);
 
     int rc = GCM_OK;
     do {
@@ -406,12 +407,74 @@ static cudaError_t launch_auto(gcm_ctx *c, int mode, int blocks, GcmParams &p, c
     DeviceGuard guard__((c)->device);                                                              \
     CU(guard__.err)
 
+// What the launch that FINISHES a message needs besides the common parameters.
+struct FinalOpts {
+    uint4 *tag_out;             // encrypt: device (or mapped host) tag
+    const uint4 *tag_in;        // decrypt: device tag, or NULL -> tag_expect
+    const uint8_t *tag_expect;  // decrypt: 16 bytes by value, or NULL
+    int *status;                // decrypt: verdict word
+    uint32_t status_init;
+};
+
+static void apply_final(GcmParams &p, const FinalOpts &f)
+{
+    if (f.tag_out) p.tag_out = f.tag_out;
+    if (f.tag_in) p.tag_in = f.tag_in;
+    if (f.tag_expect) memcpy(p.tag_expect, f.tag_expect, 16);
+    if (f.status) p.status = f.status;
+    p.status_init = f.status_init;
+}
+
+// Long aligned messages under GCM_GHASH_TENSOR: three links of a chunk chain on the caller's stream.
+//   1. AAD + the first T2_HEAD_BLOCKS payload blocks through the row kernel        -> state d_gt[0]
+//   2. whole 128-block slices through gcm_tc2_kernel (AES warps + tensor-core GHASH) -> state d_gt[1], H^(blocks of 3) -> d_gt[2]
+//   3. the rest and the length block through the row kernel, which finishes the tag / the compare
+static bool tc2_takes(const gcm_ctx *c, const void *d_in, uint64_t len, const void *d_out)
+{
+    return c->engine == GCM_GHASH_TENSOR && len >= T2_MIN_BYTES && (((uintptr_t)d_in | (uintptr_t)d_out) & 15) == 0;
+}
+
+static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const void *d_aad, uint64_t aad_len, const void *d_in,
+                            uint64_t len, void *d_out, const FinalOpts &fin, cudaStream_t s)
+{
+    const uint64_t head = 16ull * T2_HEAD_BLOCKS, nslices = (len / 16 - T2_HEAD_BLOCKS) / 128, bulk = nslices * 2048, tail = len - head - bulk;
+    const uint8_t *in = (const uint8_t *)d_in;
+    uint8_t *out = (uint8_t *)d_out;
+    GcmParams p;
+    int blocks = 0;
+    int rc = gcm_build_params(c, mode, iv, d_aad, aad_len, in, head, out, 0, false, len, aad_len, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    p.chain_out = c->d_gt + 0;
+    cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    blocks = (int)(nslices < (uint64_t)c->grid ? nslices : (uint64_t)c->grid);
+    c->ticket_next += (unsigned)blocks;
+    e = launch_tc2(c->nr, mode, blocks, c->h_rk, c->h_te0, iv, T2_HEAD_BLOCKS + 2, in + head, out + head, nslices, c->d_bmat2, c->d_hx,
+                   c->d_partials, c->d_counter, c->ticket_next - 1, c->d_gt + 0, c->d_gt + 1, (tail + 15) / 16 + 1, c->d_gt + 2, s);
+    if (e != cudaSuccess) { c->ticket_next -= (unsigned)blocks; return gcm_cuda_fail(e); }
+    rc = gcm_build_params(c, mode, iv, nullptr, 0, in + head + bulk, tail, out + head + bulk, (uint32_t)(T2_HEAD_BLOCKS + 128 * nslices), true,
+                          len, aad_len, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    p.chain_in = c->d_gt + 1;
+    p.chain_pow = c->d_gt + 2;
+    apply_final(p, fin);
+    e = gcm_launch_fused(c, mode, blocks, p, s);
+    secure_zero(&p, sizeof(p));
+    if (e != cudaSuccess) return gcm_cuda_fail(e);
+    return GCM_OK;
+}
+
 static int encrypt_async_locked(gcm_ctx *c, const uint8_t iv[12], const void *d_aad, uint64_t aad_len,
                                 const void *d_pt, uint64_t len, void *d_ct, void *d_tag, void *stream)
 {
     GcmParams p;
     int blocks = 0;
     if (!d_tag) return GCM_ERR_ARG;
+    if (iv && tc2_takes(c, d_pt, len, d_ct) && len <= ((1ull << 36) - 32) && (!aad_len || d_aad)) {
+        const FinalOpts fin = {(uint4 *)d_tag, nullptr, nullptr, nullptr, 0};
+        return crypt_tc2_locked(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, fin, (cudaStream_t)stream);
+    }
     int rc = gcm_build_params(c, MODE_ENCRYPT, iv, d_aad, aad_len, d_pt, len, d_ct, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_out = (uint4 *)d_tag;
@@ -436,6 +499,15 @@ extern "C" int gcm_decrypt_verify_async(gcm_ctx *c, const uint8_t iv[12], const 
     GcmParams p;
     int blocks = 0;
     if (!d_tag || !d_status) return GCM_ERR_ARG;
+    if (iv && tc2_takes(c, d_ct, len, d_pt) && len <= ((1ull << 36) - 32) && (!aad_len || d_aad)) {
+        CU(cudaMemsetAsync(d_status, 0x7F, 4, (cudaStream_t)stream));       // reads "refused" (non-zero) until the last link has decided
+        const FinalOpts fin = {nullptr, (const uint4 *)d_tag, nullptr, (int *)d_status, 1};
+        int rc2 = crypt_tc2_locked(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, fin, (cudaStream_t)stream);
+        if (rc2 != GCM_OK) return rc2;
+        launch_wipe((uint8_t *)d_pt, len, (const int *)d_status, (cudaStream_t)stream);
+        CU(cudaGetLastError());
+        return GCM_OK;
+    }
     int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, true, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.tag_in = (const uint4 *)d_tag;
@@ -503,17 +575,24 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
     LOCK_CTX(c);
     GcmParams p;
     int blocks = 0;
-    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, true, len, aad_len, &p, &blocks);
-    if (rc != GCM_OK) return rc;
-    memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
     // verdict written straight into mapped pinned host memory; it reads "refused" until the finisher says
     // otherwise, so a launch that never finishes cannot pass for an accepted message (fail closed)
     volatile int *verdict = (volatile int *)(c->h_pinned + 16);
+    if (iv && tc2_takes(c, d_ct, len, d_pt) && len <= ((1ull << 36) - 32) && (!aad_len || d_aad)) {
+        *verdict = GCM_STATUS_PENDING;
+        const FinalOpts fin = {nullptr, nullptr, tag, (int *)(c->h_pinned + 16), 0};
+        int rc2 = crypt_tc2_locked(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, fin, (cudaStream_t)stream);
+        if (rc2 != GCM_OK) return rc2;
+    } else {
+    int rc = gcm_build_params(c, MODE_DECRYPT, iv, d_aad, aad_len, d_ct, len, d_pt, 0, true, len, aad_len, &p, &blocks);
+    if (rc != GCM_OK) return rc;
+    memcpy(p.tag_expect, tag, 16);      // expected tag travels by value; compared on the device
     *verdict = GCM_STATUS_PENDING;
     p.status = (int *)(c->h_pinned + 16);
     cudaError_t e = launch_auto(c, MODE_DECRYPT, blocks, p, (cudaStream_t)stream);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
+    }
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     if (*verdict != 0) {
         launch_wipe((uint8_t *)d_pt, len, nullptr, (cudaStream_t)stream);

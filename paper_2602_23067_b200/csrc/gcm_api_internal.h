@@ -26,6 +26,7 @@ struct gcm_ctx {
     uint4    *d_bmat;     // bit matrices of K^0 .. K^TC_L (gcm_tc.cu)
     uint4    *d_bmat2;    // bit matrices of H^(128 e), e < GT_L, and the multiplier table of H^(128 GT_L) (gcm_ghash_tc.cu)
     uint4    *d_ktab2;
+    uint4    *d_gt;       // chain scratch of the three-launch tensor path (gcm_tc2.cu): state behind the head, behind the stretch, chain power of the tail
     uint4    *d_partials;
     unsigned *d_counter;
     uint4    *d_tag;

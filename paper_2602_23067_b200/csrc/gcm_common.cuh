@@ -45,6 +45,11 @@
 #define GT_AUTO_BYTES     (32ull << 20)  /* GCM_GHASH_AUTO: its prologue (192 KB of tables, TMEM) costs the tensor kernel about 3 us
                                             more than the table kernel; it is level at 32 MiB and ahead beyond */
 
+// AES-CTR + tensor-core GHASH with separate warps (gcm_tc2.cu): the stretch starts at payload block T2_HEAD_BLOCKS, whose
+// counter (block index + 2) is 0 mod 256, and is a whole number of 128-block slices.
+#define T2_HEAD_BLOCKS    254
+#define T2_MIN_BYTES      (8ull << 20)
+
 #define GCM_MAX_THREADS 512
 #define GCM_MAX_GRID    4096
 #define GCM_MAX_DEVICES 64
