@@ -71,12 +71,15 @@ __device__ __forceinline__ void t2_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// The helper warps spend most of their time waiting; a try_wait that comes back every few dozen cycles costs issue
+// slots and MIO bandwidth the AES warps need (105 SYNCS per warp-row were measured), so the wait carries a suspend-time
+// hint: the hardware parks the warp until the phase completes or the hint runs out.
 __device__ __forceinline__ void t2_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t done;
     do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
     } while (!done);
 }
 __device__ __forceinline__ bool t2_elect()
