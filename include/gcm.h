@@ -102,13 +102,14 @@ GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
  *   GCM_GHASH_TABLE   an 8-bit Shoup table of the stride power K = H^32 in shared memory, 16 reads of 16 bytes per
  *                     block (gcm_fused.cu), for every call;
  *   GCM_GHASH_TENSOR  the tensor cores: the multiply as a GF(2) matrix-vector product, tcgen05.mma kind::mxf4 with
- *                     0 / 1 operands, accumulators in TMEM, parity of the counts.  The single-message encrypt / decrypt /
- *                     GHASH calls run gcm_tc.cu (CTAs of 12 warps that take rows + 3 that issue the MMAs; `threads` of
- *                     gcm_set_geometry is ignored, `grid` kept), and gcm_ghash_async on at least 4 MiB of 16-byte
- *                     aligned input runs gcm_ghash_tc.cu (one launch over pad | AAD | C | length block);
- *   GCM_GHASH_AUTO    (default) what is fastest on a B200: the table for encrypt / decrypt, the tensor cores for
- *                     gcm_ghash_async on at least 32 MiB of aligned input (below that the table kernel's shorter
- *                     prologue wins).
+ *                     0 / 1 operands, accumulators in TMEM, parity of the counts.  Encrypt / decrypt of at least 8 MiB
+ *                     with 16-byte aligned buffers run gcm_tc2.cu (AES warps and tensor-core GHASH warps side by side)
+ *                     between two short launches of the row kernel (AAD and first blocks; rest and length block);
+ *                     shorter or unaligned messages run gcm_tc.cu (the row kernel with a7 on the tensor cores);
+ *                     gcm_ghash_async on at least 4 MiB of aligned input runs gcm_ghash_tc.cu.  `threads` of
+ *                     gcm_set_geometry is ignored by these kernels, `grid` kept;
+ *   GCM_GHASH_AUTO    (default) what is fastest on a B200: the tensor-core kernels for aligned messages of at least
+ *                     256 MiB (AES-128: 160 MiB) and for gcm_ghash_async on at least 32 MiB, the table otherwise.
  * Results are bit-identical under all three.  The batched calls and the latency kernel are not affected.
  * Returns GCM_OK / GCM_ERR_ARG.
  */

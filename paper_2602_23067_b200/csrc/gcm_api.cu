@@ -431,7 +431,10 @@ static void apply_final(GcmParams &p, const FinalOpts &f)
 //   3. the rest and the length block through the row kernel, which finishes the tag / the compare
 static bool tc2_takes(const gcm_ctx *c, const void *d_in, uint64_t len, const void *d_out)
 {
-    return c->engine == GCM_GHASH_TENSOR && len >= T2_MIN_BYTES && (((uintptr_t)d_in | (uintptr_t)d_out) & 15) == 0;
+    if ((((uintptr_t)d_in | (uintptr_t)d_out) & 15) != 0) return false;
+    if (c->engine == GCM_GHASH_TENSOR) return len >= T2_MIN_BYTES;
+    if (c->engine == GCM_GHASH_AUTO) return len >= (c->nr == 10 ? T2_AUTO_BYTES_128 : T2_AUTO_BYTES_256);
+    return false;
 }
 
 static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const void *d_aad, uint64_t aad_len, const void *d_in,

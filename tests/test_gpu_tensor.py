@@ -143,6 +143,67 @@ def test_tensor_engine_equals_table_engine_at_64_mib(G, oracle):
         G.gcm_destroy(ctx)
 
 
+@pytest.mark.parametrize("grid", [0, 3, 200])
+def test_tc2_chain_shapes(G, oracle, grid):
+    """gcm_tc2_kernel (AES warps + tensor-core GHASH warps) between the two row-kernel links, engine TENSOR: lengths on
+    and around the 8 MiB threshold and around whole 128-block slices behind the 254-block head (0, 1, 127 blocks and a
+    ragged byte count left for the last link), one to many chunks of 7 slices per CTA (3 CTAs: hundreds of chunks each;
+    200 CTAs: more CTAs than the SMs), AAD 0 / 16 / 2880, both key sizes, in place.  Every ciphertext byte and the tag
+    against the oracle; decrypt from oracle-written ciphertext; a forged byte inside the tensor stretch, one in the head
+    and one in the tail: refused and zero-filled."""
+    import workloads
+    rng = np.random.default_rng(9995 + grid)
+    M = 8 << 20
+    head = 254 * 16
+    lens = [M, M + 1, M - 16 + head % 2048, head + 2048 * 4096, head + 2048 * 4096 + 2047, head + 2048 * 4099 + 16 * 127 + 5, 3 * M + 777]
+    for klen in (16, 32):
+        key = rnd(rng, klen).tobytes()
+        ctx = G.gcm_init(key)
+        try:
+            G.gcm_set_geometry(ctx, grid, 0)
+            G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)
+            for i, n in enumerate(lens):
+                a = [0, 16, 2880][i % 3]
+                iv, aad, pt = rnd(rng, 12).tobytes(), rnd(rng, a), workloads.random_payload(rng, n)
+                want_ct, want_tag = oracle_encrypt(oracle, key, iv, aad, pt)
+                d_aad = dev(aad) if a else None
+                d_in = dev(pt)
+                d_out = d_in if i % 3 == 1 else torch.full((n,), 0xEE, dtype=torch.uint8, device="cuda")
+                tag = G.gcm_encrypt(ctx, iv, d_aad, d_in, d_out)
+                assert np.array_equal(d_out.cpu().numpy(), want_ct), (klen, n, a, "ciphertext")
+                assert bytes(tag) == want_tag, (klen, n, a, "tag")
+                d_ct = dev(want_ct)
+                d_pt = torch.full((n,), 0xEE, dtype=torch.uint8, device="cuda")
+                assert G.gcm_decrypt_verify(ctx, iv, d_aad, d_ct, d_pt, want_tag) == G.GCM_OK
+                assert np.array_equal(d_pt.cpu().numpy(), pt), (klen, n, a, "plaintext")
+                for pos in (7, head + 2048 * 1000 + 3, n - 1):
+                    forged = want_ct.copy()
+                    forged[pos] ^= 0x04
+                    d_pt.fill_(0xEE)
+                    assert G.gcm_decrypt_verify(ctx, iv, d_aad, dev(forged), d_pt, want_tag) == G.GCM_ERR_AUTH, (n, pos)
+                    assert not bool(d_pt.any())
+            # the asynchronous forms: device tag, device verdict word
+            n = lens[-1]
+            iv, aad, pt = rnd(rng, 12).tobytes(), rnd(rng, 33), workloads.random_payload(rng, n)
+            want_ct, want_tag = oracle_encrypt(oracle, key, iv, aad, pt)
+            d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
+            d_ct = torch.empty(n, dtype=torch.uint8, device="cuda")
+            G.gcm_encrypt_async(ctx, iv, dev(aad), dev(pt), d_ct, d_tag)
+            torch.cuda.synchronize()
+            assert d_tag.cpu().numpy().tobytes() == want_tag and np.array_equal(d_ct.cpu().numpy(), want_ct)
+            d_status = torch.full((1,), 5, dtype=torch.int32, device="cuda")
+            d_pt = torch.empty(n, dtype=torch.uint8, device="cuda")
+            G.gcm_decrypt_verify_async(ctx, iv, dev(aad), d_ct, d_pt, d_tag, d_status)
+            torch.cuda.synchronize()
+            assert int(d_status.item()) == 0 and np.array_equal(d_pt.cpu().numpy(), pt)
+            d_ct[n // 2] ^= 1
+            G.gcm_decrypt_verify_async(ctx, iv, dev(aad), d_ct, d_pt, d_tag, d_status)
+            torch.cuda.synchronize()
+            assert int(d_status.item()) != 0 and not bool(d_pt.any())
+        finally:
+            G.gcm_destroy(ctx)
+
+
 @pytest.mark.parametrize("engine", ["auto", "tensor"])
 def test_ghash_stretch_kernel_shapes(G, oracle, engine):
     """gcm_ghash_async over at least 4 MiB (engine TENSOR) / 32 MiB (default engine) of aligned input: one launch of
