@@ -149,17 +149,23 @@ def pipe_bound_gbs(key: str, nr: int, sm_count: int, sm_mhz: float, rates: dict 
                        table design (16 T-table reads per round + a 16-lookup 8-bit Shoup multiply: 16 nr + 64 lanes)
                        and the AES table reads alone with every hoistable read hoisted (16 nr - 27 + 15/8)."""
     e = load_mix(key)["per_warp_row"]
-    lanes = e["lds32"] + 2.0 * e["lds64"] + 4.0 * e["lds128"]
+    lanes = e["lds32"] + 2.0 * e["lds64"] + 4.0 * e["lds128"] + 4.0 * e.get("sts128", 0.0)
+    if key.startswith("tc2_"):
+        # AES warps + tensor-core GHASH: the tensor core reads its B operand (the bit matrices) from shared memory through the
+        # same data pipe; those wavefronts belong to no instruction, so the launch's measured total is the count that binds
+        lanes = max(lanes, e.get("shared_wavefronts_total", 0.0))
     glob = 4.0 * (e["ldg128"] + e["stg128"])
     scale = sm_count * sm_mhz * 1e6 * 16.0 / 1e9
     out = {"mix": key, "lanes_per_block": lanes, "global_lanes_per_block": glob, "cycles_per_block_per_sm": lanes / 32.0,
            "gbs": scale / (lanes / 32.0), "gbs_with_global_wavefronts": scale / ((lanes + glob) / 32.0),
-           "counts_per_block": {k: round(e[k], 3) for k in ("lds32", "lds64", "lds128", "ldg128", "stg128")},
+           "counts_per_block": {k: round(e.get(k, 0.0), 3) for k in ("lds32", "lds64", "lds128", "sts128", "ldg128", "stg128", "shared_wavefronts_total")},
            "alu_thread_instructions_per_block": e["by_pipe_warp_instructions"].get("alu"),
            "fma_thread_instructions_per_block": e["by_pipe_warp_instructions"].get("fma"),
            "thread_instructions_per_block": e["warp_instructions"]}
     if rates and rates.get("lds32") and rates.get("lds128"):
         cyc = e["lds32"] / rates["lds32"] + 2.0 * e["lds64"] / (2.0 * rates["lds128"]) + e["lds128"] / rates["lds128"]
+        if key.startswith("tc2_"):
+            cyc = lanes / rates["lds32"]          # every wavefront of the launch at the measured wavefront rate
         out["gbs_measured_rates"] = scale / cyc
     naive = 64.0 if ghash_only else 16.0 * nr + 64.0
     out["yardsticks"] = {"plain_table_design_lanes": naive, "plain_table_design_gbs": scale / (naive / 32.0)}
@@ -227,11 +233,13 @@ def step_with(ctx, aad, ct, stream, G):
     return lambda: G.gcm_ghash_async(ctx, aad, ct, d_s, stream)
 
 
-def traffic_per_launch(payload_bytes: int):
+def traffic_per_launch(payload_bytes: int, key: str = None):
     """dram bytes per launch from the committed ncu --set full capture (profiles/), scaled by size."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
         d = json.load(open(p))
+        if key:
+            d = d[key]
         return d["dram_bytes_per_payload_byte"] * payload_bytes
     except Exception:
         return None
@@ -470,6 +478,26 @@ def run_ours(args):
             e2e["frac"] = e2e["value"] / world / link["per_direction_duplex"]
             e2e["pcie"] = link
 
+    # the shared-memory table kernel on the same message, beside it (not the reported value)
+    table_engine = None
+    if rank == 0 and n >= G.TC2_AUTO_BYTES[256]:
+        G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TABLE)
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0e.record()
+        for _ in range(args.steps):
+            step()
+        t1e.record()
+        torch.cuda.synchronize()
+        tab_ms = t0e.elapsed_time(t1e) / args.steps
+        tab_gbs = n / (tab_ms * 1e-3) / 1e9
+        tpb = pipe_bound_gbs("fused_aes256_enc", 14, torch.cuda.get_device_properties(local).multi_processor_count,
+                             float(measured_peaks().get("sm_max_mhz", 1965.0)), rates)
+        table_engine = {"kernel": "gcm_fused_kernel<14, ENCRYPT, 512> (GCM_GHASH_TABLE)", "value": tab_gbs, "unit": UNIT, "ms_per_step": tab_ms,
+                        "peak": tpb["gbs"], "frac": tab_gbs / tpb["gbs"], "lanes_per_block": tpb["lanes_per_block"]}
+        G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_AUTO)
     G.gcm_destroy(ctx)
     if rank != 0:
         replicas.finish()
@@ -480,20 +508,33 @@ def run_ours(args):
     kernel_ms = statistics.mean(per)
     achieved = n / (kernel_ms * 1e-3) / 1e9
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-    pb = pipe_bound_gbs("fused_aes256_enc", 14, sm_count, sm_mhz, rates)
+    # Under the default engine an aligned message of 256 MiB and more runs as three chained launches: the row kernel over
+    # the AAD and the first 254 blocks, gcm_tc2_kernel (AES warps + tensor-core GHASH warps) over the whole 128-block
+    # slices, the row kernel over the rest and the length block.  The dominant kernel is gcm_tc2_kernel (99.7 % of a step's
+    # device time in profiles/launches_r02_c5.csv); kernel_ms is the step (its two short links included).
+    uses_tc2 = n >= G.TC2_AUTO_BYTES[256]
+    mix_key = "tc2_aes256_enc" if uses_tc2 else "fused_aes256_enc"
+    pb = pipe_bound_gbs(mix_key, 14, sm_count, sm_mhz, rates)
     roofline = roofline_dict(pb, achieved, peaks, 2)
     roofline.update({
         "peak_source": "derived (DESIGN.md section 6): %d SMs x %.0f MHz (MEASURED_PEAKS sm_max_mhz, %s) x 16 B / %.3f cycles; "
                        "lanes from %s" % (sm_count, sm_mhz, peaks["_source"], pb["cycles_per_block_per_sm"], os.path.relpath(MIX_FILE, ROOT)),
-        "traffic": traffic_per_launch(n),
+        "traffic": traffic_per_launch(n, "tc2" if uses_tc2 else None),
         "algorithmic_bytes_per_launch": 2 * n,
         "rates": {"unit": "thread-operations per SM-cycle, measured by gcm_measure_pipe_rates on this device",
                   **{k: round(v, 2) for k, v in rates.items()}},
-        "kernel": "gcm_fused_kernel<14, ENCRYPT, 512>", "kernel_ms_mean": kernel_ms,
+        "kernel": "gcm_tc2_kernel<14, ENCRYPT> (+ two short gcm_fused_kernel links)" if uses_tc2 else "gcm_fused_kernel<14, ENCRYPT, 512>",
+        "kernel_ms_mean": kernel_ms,
         "kernel_ms_median": statistics.median(per),
     })
     if clocks.get("sm_mhz"):
-        roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs("fused_aes256_enc", 14, sm_count, clocks["sm_mhz"])["gbs"]
+        roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs(mix_key, 14, sm_count, clocks["sm_mhz"])["gbs"]
+    if uses_tc2:
+        roofline["pipe"] = ("shared-memory data pipe (LSU): %.1f wavefront-lanes per 16-byte block measured for the launch (%s): AES table reads, "
+                            "the hand-over of the ciphertext to the GHASH warps, and the tensor core's reads of the bit matrices; 32 per SM-cycle. "
+                            "GHASH itself runs on tcgen05.mma kind::mxf4" % (pb["lanes_per_block"], pb["mix"]))
+        roofline["tensor_pipe"] = {"blocks_per_sm_cycle_peak": rates.get("mma_mxf4_blocks"), "note": "one GHASH block per SM-cycle available; the kernel needs 8/7 MMA-blocks per block at the AES rate: about 14 % of the pipe"}
+        roofline["table_engine"] = table_engine
 
     cpu = None
     verified = 0
@@ -522,7 +563,7 @@ def run_ours(args):
                    "parallelism": "one independent message per GPU, no collective" if world > 1 else "single GPU",
                    "verified_keystream_blocks_vs_oracle": verified},
         "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
-        "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu, "setup": setup,
+        "e2e": e2e, "gpu_launches": (3 if uses_tc2 else 1) * args.steps, "roofline": roofline, "cpu_baseline": cpu, "setup": setup,
         "ms_per_step_median": statistics.median(per), "ms_per_step_std": statistics.pstdev(per),
     }
     print(json.dumps(line))
@@ -606,6 +647,12 @@ def run_extra(args):
         gbs = steps * n / (total_ms * 1e-3) / 1e9
         key_mix = {"c5-decrypt": "fused_aes256_dec", "c5-ghash": "fused_ghash", "c5-aes128": "fused_aes128_enc", "c2": "fused_aes256_enc",
                    "c5-tensor": "fused_aes256_enc", "c5-aes128-tensor": "fused_aes128_enc"}[w]
+        tc2 = mode == "enc" and (w.endswith("-tensor") and n >= (8 << 20) or n >= G.TC2_AUTO_BYTES[128 if nr == 10 else 256])
+        if tc2:         # the default engine (or GCM_GHASH_TENSOR) took the gcm_tc2 chain for this size
+            key_mix = {"c5-decrypt": "tc2_aes256_dec", "c5-aes128": "tc2_aes128_enc", "c2": "tc2_aes256_enc",
+                       "c5-tensor": "tc2_aes256_enc", "c5-aes128-tensor": "tc2_aes128_enc"}[w]
+            launches = launches + 2         # the head and tail links of the chain
+            what += " (default engine: gcm_tc2 chain, AES warps + tensor-core GHASH)" if not w.endswith("-tensor") else ""
         pb = pipe_bound_gbs(key_mix, nr, sm_count, sm_mhz, G.gcm_measure_pipe_rates(), ghash_only=(mode == "ghash"))
         if w == "c5-ghash":
             # The default engine (GCM_GHASH_AUTO) ran: for a long aligned input that is ONE launch of gcm_ghash_tc_kernel,
@@ -628,7 +675,7 @@ def run_extra(args):
             print(json.dumps(line))
             return
         roof = roofline_dict(pb, gbs, peaks, 1 if mode == "ghash" else 2)
-        if w.endswith("-tensor"):
+        if w.endswith("-tensor") and not tc2:
             # GHASH has left the shared-memory pipe: what binds is the AES table reads alone (the second yardstick);
             # the tcgen05.st / tcgen05.ld traffic of the tensor path adds to it and is not counted here
             y = pb["yardsticks"]

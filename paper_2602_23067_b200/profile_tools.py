@@ -134,6 +134,16 @@ def mix(report: str, out: str, key: str, command: str) -> None:
     lds32 = sum(v for k, v in by_op.items() if k.startswith("LDS")) - lds128 - lds64
     ldg128 = sum(v for k, v in by_op.items() if k.startswith("LDG") and ".128" in k)
     stg128 = sum(v for k, v in by_op.items() if k.startswith("STG") and ".128" in k)
+    sts128 = sum(v for k, v in by_op.items() if k.startswith("STS") and ".128" in k)
+    # every shared-memory wavefront of the launch, whoever caused it: the instructions above, bank conflicts, and the
+    # tensor core's reads of its B operand (gcm_tc2 / gcm_tc: they show up in ncu as "bank conflict" wavefronts)
+    wf_total = 0.0
+    raw = list(csv.reader(_ncu_page(report, "raw").splitlines()))
+    if len(raw) > 2 and "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum" in raw[0]:
+        try:
+            wf_total = float(raw[2][raw[0].index("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum")])
+        except ValueError:
+            wf_total = 0.0
     # one STG.E.EF.128 (streaming store of a full row) per fast warp-row; the slow rows are a rounding error at the
     # sizes this is captured on.  GHASH-only launches store nothing: there a row is one streaming LDG.128.
     stream_st = sum(v for k, v in by_op.items() if k.startswith("STG") and ".EF" in k and ".128" in k)
@@ -146,7 +156,8 @@ def mix(report: str, out: str, key: str, command: str) -> None:
         "kernel": kernel, "command": command, "warp_rows": warp_rows,
         "per_warp_row": {
             "lds32": per_row(lds32), "lds64": per_row(lds64), "lds128": per_row(lds128),
-            "ldg128": per_row(ldg128), "stg128": per_row(stg128),
+            "ldg128": per_row(ldg128), "stg128": per_row(stg128), "sts128": per_row(sts128),
+            "shared_wavefronts_total": per_row(wf_total),
             "warp_instructions": per_row(total), "warp_instructions_issued": per_row(issued),
             "by_pipe_warp_instructions": {k: per_row(v) for k, v in sorted(by_pipe.items())},
             "shared_wavefronts": per_row(wf_shared), "shared_wavefronts_ideal": per_row(wf_shared_ideal),
