@@ -437,6 +437,17 @@ static bool tc2_takes(const gcm_ctx *c, const void *d_in, uint64_t len, const vo
     return false;
 }
 
+// a link of the chain: header-sized, so the single-CTA latency kernel takes it when it can (no tickets drawn)
+static cudaError_t launch_link(gcm_ctx *c, int mode, int blocks, const GcmParams &p, cudaStream_t s)
+{
+    const uint64_t n_ghash = (uint64_t)p.m.n_aad_blocks + (p.m.len + 15) / 16 + p.m.len_block;
+    if (n_ghash <= SMALL_MAX_BLOCKS && p.stamps == nullptr) {
+        c->ticket_next -= (unsigned)blocks;
+        return launch_small(c->nr, mode, p, s);
+    }
+    return gcm_launch_fused(c, mode, blocks, p, s);
+}
+
 static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const void *d_aad, uint64_t aad_len, const void *d_in,
                             uint64_t len, void *d_out, const FinalOpts &fin, cudaStream_t s)
 {
@@ -448,7 +459,7 @@ static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const vo
     int rc = gcm_build_params(c, mode, iv, d_aad, aad_len, in, head, out, 0, false, len, aad_len, &p, &blocks);
     if (rc != GCM_OK) return rc;
     p.chain_out = c->d_gt + 0;
-    cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s);
+    cudaError_t e = launch_link(c, mode, blocks, p, s);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     blocks = (int)(nslices < (uint64_t)c->grid ? nslices : (uint64_t)c->grid);
@@ -462,7 +473,7 @@ static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const vo
     p.chain_in = c->d_gt + 1;
     p.chain_pow = c->d_gt + 2;
     apply_final(p, fin);
-    e = gcm_launch_fused(c, mode, blocks, p, s);
+    e = launch_link(c, mode, blocks, p, s);
     secure_zero(&p, sizeof(p));
     if (e != cudaSuccess) return gcm_cuda_fail(e);
     return GCM_OK;

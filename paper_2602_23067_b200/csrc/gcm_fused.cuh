@@ -7,7 +7,8 @@
 cudaError_t launch_fused(int nr, int mode, int threads, int blocks, const GcmParams &p, cudaStream_t s);
 
 // gcm_small.cu: single-CTA latency kernel for messages of at most SMALL_MAX_BLOCKS GHASH blocks
-// (AAD blocks + payload blocks + the length block); MODE_ENCRYPT / MODE_DECRYPT only, no chunk chaining.
+// (AAD blocks + payload blocks + the length block, if any); MODE_ENCRYPT / MODE_DECRYPT only; chain_in / chain_pow /
+// chain_out of a chunk chain are honoured (the links of gcm_tc2.cu).
 #define SMALL_MAX_BLOCKS 511
 cudaError_t launch_small(int nr, int mode, const GcmParams &p, cudaStream_t s);
 

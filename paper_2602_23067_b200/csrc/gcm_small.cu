@@ -34,7 +34,8 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
     pdl_wait();             // the payload loads below come first: nothing worth overlapping ahead of them
     const uint32_t n_aad = p.m.n_aad_blocks;
     const uint32_t n_c = (uint32_t)((p.m.len + 15) / 16);
-    const uint32_t N = n_aad + n_c + 1;                       // <= SMALL_MAX_BLOCKS
+    const uint32_t N = n_aad + n_c + p.m.len_block;           // <= SMALL_MAX_BLOCKS (a link of a chunk chain may have no length block)
+    const uint32_t ctr0 = (uint32_t)p.m.base + p.m.ctr_delta; // counter of payload block 0 of this launch: 2 + its index in the message
 
     // this thread's blocks (at most two) and their weights: global loads go out before the table fill
     uint4 x[2], w[2];
@@ -50,7 +51,7 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
         if (i < n_aad) {
             const uint64_t rem = p.m.aad_len - 16ull * i;
             x[k] = load_bytes(p.m.aad + 16ull * i, rem < 16 ? (uint32_t)rem : 16u);
-        } else if (i < N - 1) {
+        } else if (i < n_aad + n_c) {
             const uint32_t g = i - n_aad;
             const uint64_t rem = p.m.len - 16ull * g;
             cbytes[k] = rem < 16 ? (uint32_t)rem : 16u;
@@ -79,7 +80,7 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
         uint4 X = x[k];
         if (cbytes[k]) {                                      // a4-a6: payload block g, counter g + 2
             const uint32_t g = i - n_aad;
-            const uint4 ks = aes_encrypt_block<NR>(p.rk, sm, lane4, make_uint4(p.iv[0], p.iv[1], p.iv[2], bswap32(g + 2u)));
+            const uint4 ks = aes_encrypt_block<NR>(p.rk, sm, lane4, make_uint4(p.iv[0], p.iv[1], p.iv[2], bswap32(g + ctr0)));
             const uint4 y = xor4(x[k], ks);
             if (cbytes[k] == 16 && p.m.aligned) st16_stream(p.m.out + 16ull * g, y);
             else store_bytes(p.m.out + 16ull * g, y, cbytes[k]);
@@ -89,6 +90,8 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
     }
     acc = cta_xor_reduce(acc, red);                           // a8 (no a9: one CTA)
     if (t == 0) {
+        if (p.chain_in != nullptr) acc = xor4(acc, gf_mul_mem(*p.chain_in, *p.chain_pow));      // a link of a chunk chain (gcm_tc2.cu)
+        if (p.chain_out != nullptr) { *p.chain_out = acc; return; }
         const uint4 tag = xor4(acc, s_ekj0);                  // a11
         if (MODE == MODE_ENCRYPT) {
             *p.tag_out = tag;
