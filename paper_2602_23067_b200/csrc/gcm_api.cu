@@ -454,6 +454,11 @@ static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const vo
     const uint64_t head = 16ull * T2_HEAD_BLOCKS, nslices = (len / 16 - T2_HEAD_BLOCKS) / 128, bulk = nslices * 2048, tail = len - head - bulk;
     const uint8_t *in = (const uint8_t *)d_in;
     uint8_t *out = (uint8_t *)d_out;
+    {   // the links only see their own stretch: the whole-message checks are made here
+        const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+        if (a != b && a < b + len && b < a + len) return GCM_ERR_ARG;            // partial overlap
+        if (aad_len >= (1ull << 61) || (aad_len + 15) / 16 > 0xFFFFFFFFull) return GCM_ERR_LEN;
+    }
     GcmParams p;
     int blocks = 0;
     int rc = gcm_build_params(c, mode, iv, d_aad, aad_len, in, head, out, 0, false, len, aad_len, &p, &blocks);

@@ -278,3 +278,19 @@ def test_ghash_stretch_kernel_4_gib(G, oracle):
     lenblk = (8 * len(aad)).to_bytes(8, "big") + (8 * n).to_bytes(8, "big")
     acc ^= np.frombuffer(oracle.ghash_segment(h, lenblk, 0), np.uint8)
     assert got == acc.tobytes()
+
+
+def test_tc2_chain_refuses_partial_overlap(G):
+    """The links of the chain check only their own stretch; a partial overlap of the whole buffers (beyond the head
+    link's 4064 bytes) must still be refused before anything is launched."""
+    n = 16 << 20
+    big = torch.zeros(n + (1 << 20), dtype=torch.uint8, device="cuda")
+    ctx = G.gcm_init(bytes(32))
+    try:
+        G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)
+        with pytest.raises(G.GcmError) as e:
+            G.gcm_encrypt(ctx, bytes(12), None, big[:n], big[65536: 65536 + n])
+        assert e.value.code == G.GCM_ERR_ARG
+        assert not bool(big.any())
+    finally:
+        G.gcm_destroy(ctx)
