@@ -145,3 +145,72 @@ def test_chunk_plan_invariants(G):
             assert plan[0] <= plan[1] <= plan[2] and plan[-1] <= plan[-2] <= plan[-3], (n, plan[:4], plan[-4:])
         assert len(plan) <= 1100
     assert len(G.gcm_debug_plan_chunks(64 * MiB)) <= 10                      # few chunks: a copy costs ~30 us on top of its bytes
+
+
+# ---- CPU model of the tensor-core GHASH: GF(2) matrix products as integer counts + parity ----------
+def _bits_mem(block: bytes) -> np.ndarray:
+    """The 128 bits of a block in the kernels' "mem" order: bit b of little-endian word i is index 32 i + b."""
+    w = np.frombuffer(block, dtype="<u4")
+    return ((w[:, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1).astype(np.int64).reshape(128)
+
+
+def _block_of_bits(bits: np.ndarray) -> bytes:
+    w = (bits.reshape(4, 32).astype(np.uint64) << np.arange(32, dtype=np.uint64)[None, :]).sum(axis=1).astype("<u4")
+    return w.tobytes()
+
+
+def _matrix_of(oracle, p: bytes) -> np.ndarray:
+    """M(P): row k = the bits of (unit block k) . P, by the oracle's bit-serial multiply."""
+    m = np.zeros((128, 128), dtype=np.int64)
+    for k in range(128):
+        u = np.zeros(128, dtype=np.int64)
+        u[k] = 1
+        m[k] = _bits_mem(oracle.gf_mul(_block_of_bits(u), p))
+    return m
+
+
+def test_model_of_the_tensor_ghash_equals_horner(oracle):
+    """What gcm_ghash_tc_kernel computes, with the ORACLE's field operations and plain integer arithmetic in place of the
+    tensor core: the virtual sequence [pad | AAD | C | length block] in whole chunks of 16 slices of 128 consecutive
+    blocks; per chunk and row j the COUNT sum_t bits(X_(128 t + j)) x M(K^(15 - t)) over the integers with the operand
+    nibbles weighted 0.5 / 1 / 2 / 2 and the matrix rows 2 / 1 / 0.5 / 0.5 (every product exactly 1), its parity as Z_j,
+    Y_j <- Y_j . K^16 xor Z_j, at the end sum_j Y_j . H^(128 - j) and the weight of the chunks behind the run.  Two CTAs
+    with different numbers of chunks.  Must equal the Horner chain of PAPER.md Eq. 1 (L191): a wrong matrix
+    orientation, bit order, weight pairing, slice power or row exponent fails here without a GPU."""
+    rng = np.random.default_rng(31337)
+    key = rng.integers(0, 256, 32, dtype=np.uint8).tobytes()
+    h = oracle.hash_subkey(key)
+    K = oracle.gf_pow(h, 128)
+    L, SL = 16, 128
+    mats = [_matrix_of(oracle, oracle.gf_pow(h, 128 * e)) for e in range(L)]
+    # e2m1 values of the operand nibbles for message bit positions 4m + j, j = 0..3, and of the matrix rows that meet them
+    a_w = np.tile(np.array([0.5, 1.0, 2.0, 2.0]), 32)
+    b_w = np.tile(np.array([2.0, 1.0, 0.5, 0.5]), 32)
+    for (n, a) in ((3 * 32768 + 5, 33), (2 * 32768 - 16 * 3, 0)):
+        aad, c = rng.integers(0, 256, a, dtype=np.uint8).tobytes(), rng.integers(0, 256, n, dtype=np.uint8).tobytes()
+        lenblk = (8 * a).to_bytes(8, "big") + (8 * n).to_bytes(8, "big")
+        real = blocks_of(aad) + blocks_of(c) + [lenblk]
+        nchunks = (len(real) + L * SL - 1) // (L * SL)
+        X = [ZERO] * (nchunks * L * SL - len(real)) + real                 # leading zero blocks are free
+        total = ZERO
+        cuts = [0, nchunks // 2, nchunks] if nchunks > 1 else [0, nchunks]
+        for c0, c1 in zip(cuts[:-1], cuts[1:]):                             # one "CTA" per run of chunks
+            Y = [ZERO] * SL
+            for ch in range(c0, c1):
+                counts = np.zeros((SL, 128))
+                for t in range(L):
+                    rows = np.stack([_bits_mem(X[(ch * L + t) * SL + j]) for j in range(SL)]).astype(np.float64)
+                    counts += (rows * a_w[None, :]) @ (mats[L - 1 - t] * b_w[:, None])
+                assert np.all(counts == np.floor(counts)) and counts.max() < 2 ** 24
+                Z = [_block_of_bits((counts[j].astype(np.int64) & 1)) for j in range(SL)]
+                KL = oracle.gf_pow(h, 128 * L)
+                Y = [xor(oracle.gf_mul(Y[j], KL), Z[j]) for j in range(SL)]
+            part = ZERO
+            for j in range(SL):
+                part = xor(part, oracle.gf_mul(Y[j], oracle.gf_pow(h, 128 - j)))
+            behind = (nchunks - c1) * L * SL
+            if behind:
+                part = oracle.gf_mul(part, oracle.gf_pow(h, behind))
+            total = xor(total, part)
+        assert total == oracle.ghash(h, aad, c), (n, a)
+    assert K == oracle.gf_pow(oracle.gf_pow(h, 64), 2)
