@@ -294,3 +294,32 @@ def test_tc2_chain_refuses_partial_overlap(G):
         assert not bool(big.any())
     finally:
         G.gcm_destroy(ctx)
+
+
+@pytest.mark.parametrize("klen", [16, 32])
+def test_default_engine_switches_at_its_threshold(G, oracle, klen):
+    """GCM_GHASH_AUTO: an aligned message of exactly the threshold size (AES-128: 192 MiB, AES-256: 384 MiB) takes the
+    gcm_tc2 chain, one block less the table kernel; both against the oracle (every ciphertext byte, the tag by the
+    pinned segment identity), and the two ciphertexts agree on their common prefix."""
+    import workloads
+    rng = np.random.default_rng(9996 + klen)
+    n = G.TC2_AUTO_BYTES[8 * klen]
+    key, iv, aad = rnd(rng, klen).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, 2880)
+    pt = workloads.random_payload(rng, n)
+    ref = oracle.ctr_xor(key, iv, pt, threads=THREADS)
+    h, ek = oracle.hash_subkey(key), oracle.ek_j0(key, iv)
+    ctx = G.gcm_init(key)
+    try:
+        assert G.gcm_get_ghash_engine(ctx) == G.GCM_GHASH_AUTO
+        d_pt, d_aad = dev(pt), dev(aad)
+        for m in (n, n - 16):
+            d_ct = torch.full((m,), 0xEE, dtype=torch.uint8, device="cuda")
+            tag = G.gcm_encrypt(ctx, iv, d_aad, d_pt[:m], d_ct)
+            assert np.array_equal(d_ct.cpu().numpy(), ref[:m]), (klen, m, "ciphertext")
+            s = oracle.ghash_segmented(h, aad, ref[:m], 1 << 16, THREADS)
+            assert bytes(tag) == bytes(x ^ y for x, y in zip(s, ek)), (klen, m, "tag")
+            d_back = torch.empty(m, dtype=torch.uint8, device="cuda")
+            assert G.gcm_decrypt_verify(ctx, iv, d_aad, d_ct, d_back, tag) == G.GCM_OK
+            assert torch.equal(d_back, d_pt[:m])
+    finally:
+        G.gcm_destroy(ctx)
