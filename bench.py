@@ -841,6 +841,7 @@ def run_extra(args):
         aad = torch.from_numpy(m.aad).cuda()
         d_tag = torch.zeros(16, dtype=torch.uint8, device="cuda")
         pb = pipe_bound_gbs("fused_aes256_enc", 14, sm_count, sm_mhz)
+        pb2 = pipe_bound_gbs("tc2_aes256_enc", 14, sm_count, sm_mhz)      # from 384 MiB on the default engine runs the gcm_tc2 chain
         out = {}
         for mib in (1, 4, 16, 64, 256, 1024):
             n = mib << 20
@@ -861,7 +862,9 @@ def run_extra(args):
                 torch.cuda.synchronize()
                 us = e0.elapsed_time(e1) * 1e3 / reps
                 best = us if best is None else min(best, us)
-            out["%d_MiB" % mib] = {"us_per_launch": best, "GBps": n / best / 1e3, "frac_of_pipe_bound": n / best / 1e3 / pb["gbs"]}
+            tc2 = n >= G.TC2_AUTO_BYTES[256]
+            out["%d_MiB" % mib] = {"us_per_launch": best, "GBps": n / best / 1e3, "kernel": "gcm_tc2 chain" if tc2 else "gcm_fused_kernel",
+                                   "pipe_bound_gbs": (pb2 if tc2 else pb)["gbs"], "frac_of_pipe_bound": n / best / 1e3 / (pb2 if tc2 else pb)["gbs"]}
             del pts, cts
         G.gcm_destroy(ctx)
         line.update(metric="AES-256-GCM encrypt GB/s by message size (device-timed trains of launches)",
