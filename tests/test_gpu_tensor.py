@@ -323,3 +323,35 @@ def test_default_engine_switches_at_its_threshold(G, oracle, klen):
             assert torch.equal(d_back, d_pt[:m])
     finally:
         G.gcm_destroy(ctx)
+
+
+def test_tc2_chain_random_shapes(G, oracle):
+    """40 seeded random shapes through the gcm_tc2 chain (engine TENSOR): lengths 8 .. 24 MiB with any byte count, AAD of
+    0 .. 6000 bytes (above 4 KB the head link no longer fits the latency kernel and runs on the row kernel), random grid,
+    key size, encrypt or decrypt; every byte and the tag against the oracle."""
+    import workloads
+    rng = np.random.default_rng(9997)
+    for i in range(40):
+        klen = 16 if rng.integers(0, 2) else 32
+        n = int(rng.integers(8 << 20, 24 << 20))
+        a = int(rng.integers(0, 6001)) if i % 4 else 0
+        grid = int(rng.choice([0, 0, 1, 17, 148, 400]))
+        key, iv, aad = rnd(rng, klen).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, a)
+        pt = workloads.random_payload(rng, n)
+        want_ct, want_tag = oracle_encrypt(oracle, key, iv, aad, pt)
+        ctx = G.gcm_init(key)
+        try:
+            G.gcm_set_geometry(ctx, grid, 0)
+            G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)
+            d_aad = dev(aad) if a else None
+            if i % 2 == 0:
+                d_ct = torch.empty(n, dtype=torch.uint8, device="cuda")
+                tag = G.gcm_encrypt(ctx, iv, d_aad, dev(pt), d_ct)
+                assert np.array_equal(d_ct.cpu().numpy(), want_ct), (i, klen, n, a, grid, "ciphertext")
+                assert bytes(tag) == want_tag, (i, klen, n, a, grid, "tag")
+            else:
+                d_pt = torch.empty(n, dtype=torch.uint8, device="cuda")
+                assert G.gcm_decrypt_verify(ctx, iv, d_aad, dev(want_ct), d_pt, want_tag) == G.GCM_OK, (i, klen, n, a, grid)
+                assert np.array_equal(d_pt.cpu().numpy(), pt), (i, klen, n, a, grid, "plaintext")
+        finally:
+            G.gcm_destroy(ctx)
