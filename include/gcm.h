@@ -109,7 +109,7 @@ GCM_API int gcm_get_geometry(const gcm_ctx *ctx, int *grid, int *threads);
  *                     gcm_ghash_async on at least 4 MiB of aligned input runs gcm_ghash_tc.cu.  `threads` of
  *                     gcm_set_geometry is ignored by these kernels, `grid` kept;
  *   GCM_GHASH_AUTO    (default) what is fastest on a B200: the tensor-core kernels for aligned messages of at least
- *                     384 MiB (AES-128: 192 MiB) and for gcm_ghash_async on at least 32 MiB, the table otherwise.
+ *                     384 MiB (AES-128: 128 MiB) and for gcm_ghash_async on at least 32 MiB, the table otherwise.
  * Results are bit-identical under all three.  The batched calls and the latency kernel are not affected.
  * Returns GCM_OK / GCM_ERR_ARG.
  */

@@ -49,8 +49,8 @@
 // counter (block index + 2) is 0 mod 256, and is a whole number of 128-block slices.
 #define T2_HEAD_BLOCKS    254
 #define T2_MIN_BYTES      (8ull << 20)      /* GCM_GHASH_TENSOR: from here on gcm_tc2.cu, below it gcm_tc.cu */
-#define T2_AUTO_BYTES_256 (384ull << 20)    /* GCM_GHASH_AUTO: the two extra launches of the chain cost about 19 us; level with the */
-#define T2_AUTO_BYTES_128 (192ull << 20)    /* table kernel at 256 MiB (AES-256) / 150 MiB (AES-128), ahead beyond */
+#define T2_AUTO_BYTES_256 (384ull << 20)    /* GCM_GHASH_AUTO: a chain costs 25-30 us more than it would at its steady rate; level with */
+#define T2_AUTO_BYTES_128 (128ull << 20)    /* the table kernel at 230 MiB (AES-256) / 96 MiB (AES-128), ahead beyond */
 
 #define GCM_MAX_THREADS 512
 #define GCM_MAX_GRID    4096

@@ -41,7 +41,7 @@
 #define T2_BMAT_OFF  AES_TAB_BYTES
 #define T2_STAGE_OFF (T2_BMAT_OFF + (T2_L + 1) * TC_BMAT_BYTES)
 #define T2_RED_OFF   (T2_STAGE_OFF + T2_STAGES * 2048)
-#define T2_BAR_OFF   (T2_RED_OFF + 64)               /* tabbar, sfull[16], sempty[16], tfull[12], tempty[12], yfull[2], accfull[2] */
+#define T2_BAR_OFF   (T2_RED_OFF + 128)              /* tabbar, sfull[16], sempty[16], tfull[12], tempty[12], yfull[2], accfull[2] */
 #define T2_SMEM_BYTES (T2_BAR_OFF + 64 * 8 + 16)
 #define T2_IDESC ((1u << 7) | (1u << 10) | (16u << 17) | (1u << 23) | (8u << 24))
 static_assert(T2_L + 1 <= GT_L, "the matrices of H^(128 e), e <= T2_L, come from the GHASH-only kernel's set");
@@ -256,6 +256,12 @@ gcm_tc2_kernel(const __grid_constant__ Tc2Params p)
         const uint32_t lanebase = tb + ((32u * q) << 16);
         const uint32_t mine = stage0 + 512 * q + 16 * lane;
         uint4 Y = make_uint4(0, 0, 0, 0);
+        // the three powers of H the finish needs, worked out now, while the first slices are still being encrypted: the
+        // weight of this CTA's run, and (used by whichever CTA draws the last ticket) those of the chained state
+        if (lane == 0 && q < 3) {
+            const uint64_t e = q == 0 ? (p.nslices - s1) * 128 : q == 1 ? p.nslices * 128 : p.exp_next;
+            red[4 + q] = t2_pow(p.hx, e);
+        }
         uint32_t c = 0, s_in = 0, left = T, ell = left < T2_L ? left : T2_L, slot = 0, ph = 1;
         for (uint32_t tt = 0; tt < T; tt++) {
             const uint32_t sg = tt & (T2_STAGES - 1);
@@ -344,7 +350,7 @@ gcm_tc2_kernel(const __grid_constant__ Tc2Params p)
     if (lane == 0) {
         uint4 acc = xor4(xor4(red[0], red[1]), xor4(red[2], red[3]));
         const uint64_t behind = (p.nslices - s1) * 128;
-        if (behind && T) acc = gf_mul_mem(acc, t2_pow(p.hx, behind));
+        if (behind && T) acc = gf_mul_mem(acc, red[4]);
         pdl_wait();
         p.partials[blockIdx.x] = acc;
         asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(p.counter) : "memory");
@@ -355,9 +361,9 @@ gcm_tc2_kernel(const __grid_constant__ Tc2Params p)
     for (uint32_t j = lane; j < gridDim.x; j += 32) tot = xor4(tot, __ldcg(p.partials + j));
     tot = t2_warp_xor4(tot);
     if (lane == 0) {
-        if (p.chain_in != nullptr) tot = xor4(tot, gf_mul_mem(*p.chain_in, t2_pow(p.hx, p.nslices * 128)));
+        if (p.chain_in != nullptr) tot = xor4(tot, gf_mul_mem(*p.chain_in, red[5]));
         *p.chain_out = tot;
-        if (p.pow_out != nullptr) *p.pow_out = t2_pow(p.hx, p.exp_next);
+        if (p.pow_out != nullptr) *p.pow_out = red[6];
     }
 }
 

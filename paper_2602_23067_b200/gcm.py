@@ -17,7 +17,7 @@ GCM_GHASH_TABLE = 0
 GCM_GHASH_TENSOR = 1
 GCM_GHASH_AUTO = 2
 # sizes from which GCM_GHASH_AUTO takes the tensor-core kernels (csrc/gcm_common.cuh: T2_AUTO_BYTES_*, GT_AUTO_BYTES)
-TC2_AUTO_BYTES = {128: 192 << 20, 256: 384 << 20}
+TC2_AUTO_BYTES = {128: 128 << 20, 256: 384 << 20}
 GHASH_TC_AUTO_BYTES = 32 << 20
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -298,7 +298,7 @@ def test_tc2_chain_refuses_partial_overlap(G):
 
 @pytest.mark.parametrize("klen", [16, 32])
 def test_default_engine_switches_at_its_threshold(G, oracle, klen):
-    """GCM_GHASH_AUTO: an aligned message of exactly the threshold size (AES-128: 192 MiB, AES-256: 384 MiB) takes the
+    """GCM_GHASH_AUTO: an aligned message of exactly the threshold size (AES-128: 128 MiB, AES-256: 384 MiB) takes the
     gcm_tc2 chain, one block less the table kernel; both against the oracle (every ciphertext byte, the tag by the
     pinned segment identity), and the two ciphertexts agree on their common prefix."""
     import workloads
