@@ -378,22 +378,43 @@ def _pack_msgs(msgs: Iterable[dict], decrypt: bool):
     return arr, len(msgs), keep
 
 
-def gcm_encrypt_batch(msgs: Iterable[dict], stream=None) -> List[bytes]:
-    """msgs: dicts with key, iv, aad (device or None), input, output (device).  Returns the tags."""
-    arr, n, keep = _pack_msgs(msgs, decrypt=False)
-    _check(_L.gcm_encrypt_batch(arr, n, _stream(stream)), "gcm_encrypt_batch")
-    del keep
-    return [bytes(arr[i].tag) for i in range(n)]
+class MsgBatch:
+    """The gcm_msg array of include/gcm.h, built once from a list of dicts (gcm_pack_msgs) so that a batch which is
+    submitted many times pays the Python-side marshalling once.  Keeps the key buffers (and nothing else) alive: the
+    device buffers the descriptors point to stay the caller's."""
+
+    def __init__(self, msgs: Iterable[dict], decrypt: bool):
+        self.decrypt = bool(decrypt)
+        self.arr, self.n, self._keep = _pack_msgs(msgs, decrypt)
+
+    def __len__(self) -> int:
+        return self.n
 
 
-def gcm_decrypt_verify_batch(msgs: Iterable[dict], stream=None) -> List[int]:
-    """msgs as above plus `tag`.  Returns the per-message status list (GCM_OK / GCM_ERR_AUTH)."""
-    arr, n, keep = _pack_msgs(msgs, decrypt=True)
-    rc = _L.gcm_decrypt_verify_batch(arr, n, _stream(stream))
+def gcm_pack_msgs(msgs: Iterable[dict], decrypt: bool = False) -> MsgBatch:
+    """dicts with key, iv, aad (device or None), input, output (device) and, for decrypt, tag -> MsgBatch."""
+    return MsgBatch(msgs, decrypt)
+
+
+def gcm_encrypt_batch(msgs, stream=None) -> List[bytes]:
+    """msgs: dicts with key, iv, aad (device or None), input, output (device), or a MsgBatch.  Returns the tags."""
+    b = msgs if isinstance(msgs, MsgBatch) else MsgBatch(msgs, decrypt=False)
+    if b.decrypt:
+        raise ValueError("a MsgBatch packed for decrypt was passed to gcm_encrypt_batch")
+    _check(_L.gcm_encrypt_batch(b.arr, b.n, _stream(stream)), "gcm_encrypt_batch")
+    return [bytes(b.arr[i].tag) for i in range(b.n)]
+
+
+def gcm_decrypt_verify_batch(msgs, stream=None) -> List[int]:
+    """msgs as above plus `tag` (or a MsgBatch packed with decrypt=True).  Returns the per-message status list
+    (GCM_OK / GCM_ERR_AUTH)."""
+    b = msgs if isinstance(msgs, MsgBatch) else MsgBatch(msgs, decrypt=True)
+    if not b.decrypt:
+        raise ValueError("a MsgBatch packed for encrypt was passed to gcm_decrypt_verify_batch")
+    rc = _L.gcm_decrypt_verify_batch(b.arr, b.n, _stream(stream))
     if rc < 0:
         raise GcmError(rc, "gcm_decrypt_verify_batch")
-    del keep
-    return [arr[i].status for i in range(n)]
+    return [b.arr[i].status for i in range(b.n)]
 
 
 GCM_DMSG_BYTES = 112

@@ -140,6 +140,30 @@ def test_batch_only_large_aes128_many_messages(G, oracle):
     G.gcm_batch_release()
 
 
+def test_batch_packed_once_submitted_twice(G, oracle):
+    """gcm_pack_msgs: the gcm_msg array is built once and handed to the C call as is; submitting it a second time after
+    the inputs changed must encrypt the new inputs (the array holds pointers, not data), and a batch packed for one
+    direction is refused by the other."""
+    rng = np.random.default_rng(9911)
+    specs = [(rnd(rng, 16 + 16 * (i % 2)).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, 5 * i), rnd(rng, n), 0, 0, False)
+             for i, n in enumerate([0, 1, 4097, LARGE + 3, 2 * LARGE])]
+    batch, outs = build_batch(specs)
+    packed = G.gcm_pack_msgs(batch)
+    assert len(packed) == len(specs)
+    for rep in range(2):
+        tags = G.gcm_encrypt_batch(packed)
+        for i, ((big_out, oo, n, _), spec, tag) in enumerate(zip(outs, specs, tags)):
+            pt = spec[3] if rep == 0 else spec[3] ^ np.uint8(0x5A)
+            ref_ct, ref_tag = oracle.gcm_encrypt(spec[0], spec[1], spec[2], pt)
+            assert tag == ref_tag, (rep, i)
+            assert np.array_equal(big_out[oo: oo + n].cpu().numpy(), ref_ct), (rep, i)
+        for b in batch:
+            b["input"] ^= 0x5A
+    with pytest.raises(ValueError):
+        G.gcm_decrypt_verify_batch(packed)
+    G.gcm_batch_release()
+
+
 @pytest.mark.parametrize("geometry", [(0, 0), (5, 256), (37, 384)])
 def test_ghash_only_shapes(G, oracle, geometry):
     """gcm_ghash_async (MODE_GHASH) on (a, len) in {0, 1, 16, 17, 2880} x {0, 1, 15, 16, 8191, 16*512*5+9}: empty A,
