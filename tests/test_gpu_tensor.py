@@ -355,3 +355,51 @@ def test_tc2_chain_random_shapes(G, oracle):
                 assert np.array_equal(d_pt.cpu().numpy(), pt), (i, klen, n, a, grid, "plaintext")
         finally:
             G.gcm_destroy(ctx)
+
+
+def test_tensor_kernels_of_several_contexts_on_several_streams(G, oracle):
+    """Three contexts (own keys, own scratch and chain slots) on three streams at the same time, all asynchronous: two run
+    gcm_tc2 chains (encrypt, then decrypt of what was just written), the third the GHASH-only tensor kernel, three rounds
+    without a host synchronisation in between.  Every kernel of these paths takes all 512 TMEM columns of its SM and most
+    of its shared memory, so CTAs of different launches queue for SMs; results must not depend on how they interleave."""
+    import workloads
+    rng = np.random.default_rng(4242)
+    n = (9 << 20) + 48
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    jobs = []
+    for j in range(3):
+        key = rnd(rng, 32 if j != 1 else 16).tobytes()
+        ctx = G.gcm_init(key)
+        G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)
+        rounds = []
+        for r in range(3):
+            iv, aad, pt = rnd(rng, 12).tobytes(), rnd(rng, 100 * j + r), workloads.random_payload(rng, n)
+            rounds.append({"iv": iv, "aad": aad, "pt": pt, "d_aad": dev(aad) if len(aad) else None, "d_pt": dev(pt),
+                           "d_ct": torch.empty(n, dtype=torch.uint8, device="cuda"), "d_back": torch.empty(n, dtype=torch.uint8, device="cuda"),
+                           "d_tag": torch.zeros(16, dtype=torch.uint8, device="cuda"), "d_status": torch.full((1,), 9, dtype=torch.int32, device="cuda"),
+                           "d_gh": torch.zeros(16, dtype=torch.uint8, device="cuda")})
+        jobs.append((key, ctx, rounds))
+    torch.cuda.synchronize()
+    try:
+        for r in range(3):
+            for j, (key, ctx, rounds) in enumerate(jobs):
+                x = rounds[r]
+                if j < 2:
+                    G.gcm_encrypt_async(ctx, x["iv"], x["d_aad"], x["d_pt"], x["d_ct"], x["d_tag"], stream=streams[j])
+                    G.gcm_decrypt_verify_async(ctx, x["iv"], x["d_aad"], x["d_ct"], x["d_back"], x["d_tag"], x["d_status"], stream=streams[j])
+                else:
+                    G.gcm_ghash_async(ctx, x["d_aad"], x["d_pt"], x["d_gh"], stream=streams[j])
+        torch.cuda.synchronize()
+        for j, (key, ctx, rounds) in enumerate(jobs):
+            for r, x in enumerate(rounds):
+                if j < 2:
+                    want_ct, want_tag = oracle_encrypt(oracle, key, x["iv"], x["aad"], x["pt"])
+                    assert np.array_equal(x["d_ct"].cpu().numpy(), want_ct), (j, r)
+                    assert x["d_tag"].cpu().numpy().tobytes() == want_tag, (j, r)
+                    assert int(x["d_status"].item()) == 0 and torch.equal(x["d_back"], x["d_pt"]), (j, r)
+                else:
+                    h = oracle.hash_subkey(key)
+                    assert x["d_gh"].cpu().numpy().tobytes() == bytes(oracle.ghash_segmented(h, x["aad"], x["pt"], 1 << 16, THREADS)), (j, r)
+    finally:
+        for _, ctx, _ in jobs:
+            G.gcm_destroy(ctx)
