@@ -510,7 +510,7 @@ def run_ours(args):
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     # Under the default engine an aligned message of 256 MiB and more runs as three chained launches: the row kernel over
     # the AAD and the first 254 blocks, gcm_tc2_kernel (AES warps + tensor-core GHASH warps) over the whole 128-block
-    # slices, the row kernel over the rest and the length block.  The dominant kernel is gcm_tc2_kernel (99.7 % of a step's
+    # slices, the row kernel over the rest and the length block.  The dominant kernel is gcm_tc2_kernel (99.8 % of a step's
     # device time in profiles/launches_r02_c5.csv); kernel_ms is the step (its two short links included).
     uses_tc2 = n >= G.TC2_AUTO_BYTES[256]
     mix_key = "tc2_aes256_enc" if uses_tc2 else "fused_aes256_enc"
