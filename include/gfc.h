@@ -112,6 +112,35 @@ GCM_API int gfc_datasum(const void *d_data, uint64_t len, uint32_t *sum, void *c
  */
 GCM_API int gfc_datasum_async(const void *d_data, uint64_t len, void *d_acc, void *cuda_stream);
 
+/*
+ * gfc_datasum_noalloc -- the DATASUM of gfc_datasum for callers that cannot allocate device memory.
+ *
+ * gfc_datasum calls cudaMalloc and cudaFree for its accumulator on every call.  That rules it out (a) in a
+ * process where something else already holds all of the GPU's memory (a framework's caching allocator, a
+ * serving engine's pre-reserved pools: a raw cudaMalloc fails there) and (b) in a latency-sensitive loop that
+ * runs beside other streams, because cudaMalloc / cudaFree may wait for the whole device.  This entry point
+ * calls neither, nor any other allocating routine: its scratch is a 128.25 KiB array that is part of the
+ * library's device image, so every GPU the library is used on holds those 128.25 KiB until the process exits.
+ *
+ *   d_data       device, len bytes, 16-byte aligned (may be NULL when len = 0)
+ *   len          at most GFC_DATASUM_NOALLOC_MAX_BYTES (4 GiB: the array holds one partial sum per 256 KiB
+ *                tile, 16384 of them); a longer buffer returns GCM_ERR_LEN and enqueues nothing -- sum it in
+ *                pieces with gfc_datasum_async instead
+ *   d_sum        device, out: one uint32, 4-byte aligned, the caller's own memory; written by the kernel
+ *   cuda_stream  the work (an 8-byte memset of the scratch's counter + one kernel) is enqueued here; the call
+ *                does not synchronise: read *d_sum after the stream has reached that point
+ *
+ * The data must live on the calling thread's current device.  The first call on each device looks up the
+ * scratch's device address (and makes the CUDA runtime load the library's module there if it has not yet):
+ * make that call once at start-up, outside any stream capture and outside the latency-critical part.
+ * All calls on one device share the one array: two calls whose kernels may run at the same time (two streams
+ * with no ordering between them, two host threads) corrupt each other's sums.  Calls that follow each other on
+ * one stream, or that are ordered by events, are safe; nothing has to be cleared between them.
+ * Returns GCM_OK / GCM_ERR_ARG (NULL or misaligned pointer) / GCM_ERR_LEN / GCM_ERR_CUDA.
+ */
+#define GFC_DATASUM_NOALLOC_MAX_BYTES (1ull << 32)
+GCM_API int gfc_datasum_noalloc(const void *d_data, uint64_t len, uint32_t *d_sum, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

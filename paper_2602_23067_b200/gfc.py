@@ -18,7 +18,8 @@ GFC_ERR_FORMAT, GFC_ERR_CAPACITY = -5, -6
 GFC_FULL_ACCESS, GFC_HEADER_FALLBACK, GFC_PAYLOAD_SUPPRESSED = 0, 1, 2
 
 EXPORTED_SYMBOLS = ["gfc_context_create", "gfc_context_destroy", "gfc_encrypt_frame", "gfc_decrypt_frame", "gfc_datasum",
-                    "gfc_datasum_async"]
+                    "gfc_datasum_async", "gfc_datasum_noalloc"]
+GFC_DATASUM_NOALLOC_MAX_BYTES = 1 << 32
 
 
 class FitsOperationResult(ctypes.Structure):
@@ -44,6 +45,7 @@ _L.gfc_encrypt_frame.argtypes = [_vp, _vp, _u64, ctypes.c_char_p, ctypes.c_char_
 _L.gfc_decrypt_frame.argtypes = [_vp, _vp, _u64, ctypes.c_char_p, ctypes.c_char_p, _ci, ctypes.POINTER(FitsOperationResult)]
 _L.gfc_datasum.argtypes = [_vp, _u64, ctypes.POINTER(ctypes.c_uint32), _vp]
 _L.gfc_datasum_async.argtypes = [_vp, _u64, _vp, _vp]
+_L.gfc_datasum_noalloc.argtypes = [_vp, _u64, _vp, _vp]
 
 
 class FrameError(GcmError):
@@ -139,3 +141,22 @@ def gfc_datasum_async(d_data, d_acc, stream=None) -> None:
     ptr, n = _gcm._dev(d_data)
     acc, _ = _gcm._dev(d_acc)
     _gcm._check(_L.gfc_datasum_async(ptr, n, acc, _gcm._stream(stream)), "gfc_datasum_async")
+
+
+def gfc_datasum_noalloc(d_data, d_sum, stream=None) -> None:
+    """DATASUM of a device buffer of at most 4 GiB without any device allocation inside the library.
+
+    For programs in which the library may not call cudaMalloc: the GPU's memory is already owned by a caching
+    allocator or a pre-reserved pool (a raw allocation would fail), or the call sits in a latency-critical loop
+    beside other streams (cudaMalloc / cudaFree can stall the whole device).  The library's own scratch for this
+    call is a fixed 128.25 KiB array inside its device image.
+
+    d_sum: device tensor of 4 bytes (one uint32 / int32) owned by the caller; written asynchronously on
+    `stream`, so synchronise (or order a later read on the same stream) before looking at it.  One call at a
+    time per GPU: calls that could overlap on the device share the scratch and would corrupt each other.
+    Raises GcmError(GCM_ERR_LEN) for more than GFC_DATASUM_NOALLOC_MAX_BYTES."""
+    ptr, n = _gcm._dev(d_data)
+    out, n_out = _gcm._dev(d_sum)
+    if n_out != 4:
+        raise ValueError("d_sum must be a device buffer of exactly 4 bytes")
+    _gcm._check(_L.gfc_datasum_noalloc(ptr, n, out, _gcm._stream(stream)), "gfc_datasum_noalloc")

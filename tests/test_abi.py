@@ -40,7 +40,7 @@ def test_binding_lists_the_same_symbols(lib_path):
     assert pkg.library_path() == lib_path
     from paper_2602_23067_b200 import gfc
     assert sorted(gfc.EXPORTED_SYMBOLS) == declared_symbols("gfc.h", "gfc_")
-    assert len(gfc.EXPORTED_SYMBOLS) == 6
+    assert len(gfc.EXPORTED_SYMBOLS) == 7
 
 
 def test_argument_errors_without_gpu(lib_path):
