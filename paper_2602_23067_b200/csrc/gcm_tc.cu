@@ -299,6 +299,21 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
     tc_fence_after();
     const uint32_t tbase = *tslot;
 
+    // Scale factors (every byte 2^0, UE8M0 127) go into TMEM between two CTA barriers, as in gcm_tc2.cu: the issuing
+    // warps wait only on the matrix copy and on the producers' full[] arrivals, and a warp whose run is short arrives
+    // almost at once, so without the second barrier an MMA of group 1 or 2 could read column TC_COL_SF before the
+    // quarter warps' tcgen05.st has landed there.
+    if (warp < 4) {
+        const uint32_t one = 0x7F7F7F7Fu, a = tbase + ((32u * warp) << 16) + TC_COL_SF;
+#pragma unroll
+        for (int c = 0; c < 32; c += 8)
+            asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(a + c), "r"(one) : "memory");
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();                                    // scale factors are in TMEM before any MMA can be issued
+    tc_fence_after();
+
     if (warp >= TC_NW) {
         // ---- the issuing warp of group g: its slices in order.  Every lane walks the loop, so that addresses and
         // descriptors are warp-uniform and sit in uniform registers (UTCOMMA takes no others; from a single lane of a
@@ -341,13 +356,6 @@ gcm_tc_kernel(const __grid_constant__ GcmParams p)
     }
 
     // ---- producer warps ---------------------------------------------------------------------------------------
-    if (warp < 4) {                                     // scale factors: every byte 2^0 (UE8M0 127)
-        const uint32_t one = 0x7F7F7F7Fu, a = tbase + ((32u * warp) << 16) + TC_COL_SF;
-#pragma unroll
-        for (int c = 0; c < 32; c += 8)
-            asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(a + c), "r"(one) : "memory");
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-    }
     if (warp == 0) tc_position_weights(p, lane, wpow);
 
     CtrConst cc = {0, 0, 0, 0};
