@@ -32,6 +32,8 @@ gcm_small_kernel(const __grid_constant__ GcmParams p)
 
     pdl_launch_dependents();
     pdl_wait();             // the payload loads below come first: nothing worth overlapping ahead of them
+    // fail closed, as in gcm_fused.cu: a device-resident verdict word reads "refused" until thread 0 has compared the tags
+    if (MODE == MODE_DECRYPT && p.status_init && t == 0 && p.chain_out == nullptr) *p.status = GCM_STATUS_PENDING;
     const uint32_t n_aad = p.m.n_aad_blocks;
     const uint32_t n_c = (uint32_t)((p.m.len + 15) / 16);
     const uint32_t N = n_aad + n_c + p.m.len_block;           // <= SMALL_MAX_BLOCKS (a link of a chunk chain may have no length block)

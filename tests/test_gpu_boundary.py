@@ -142,6 +142,32 @@ def test_async_verdict_fails_closed_and_is_rewritten_every_call(G, oracle):
         G.gcm_destroy(ctx)
 
 
+@pytest.mark.parametrize("n", [1, 100, 16 * 509, 8000])
+def test_async_verdict_of_header_sized_messages(G, oracle, n):
+    """The same contract for messages of at most 511 GHASH blocks, which the default geometry sends to the one-CTA
+    latency kernel (gcm_small.cu): that kernel too overwrites a stale verdict, in both directions."""
+    rng = np.random.default_rng(9980 + n)
+    for key_bytes in (16, 32):
+        key, iv, aad = rnd(rng, key_bytes).tobytes(), rnd(rng, 12).tobytes(), rnd(rng, 21).tobytes()
+        pt = rnd(rng, n)
+        ct, tag = oracle.gcm_encrypt(key, iv, aad, pt)
+        ctx = G.gcm_init(key)
+        try:
+            d_ct, d_tag, d_aad = dev(ct), dev(np.frombuffer(tag, np.uint8)), dev(np.frombuffer(aad, np.uint8))
+            out = torch.full((n,), 0xAA, dtype=torch.uint8, device="cuda")
+            d_status = torch.zeros(1, dtype=torch.int32, device="cuda")       # stale "accepted"
+            bad = d_ct.clone(); bad[n // 2] ^= 0x80
+            G.gcm_decrypt_verify_async(ctx, iv, d_aad, bad, out, d_tag, d_status)
+            torch.cuda.synchronize()
+            assert int(d_status.item()) == G.GCM_ERR_AUTH and not bool(out.any().item())
+            d_status.fill_(1)                                                   # stale "refused"
+            G.gcm_decrypt_verify_async(ctx, iv, d_aad, d_ct, out, d_tag, d_status)
+            torch.cuda.synchronize()
+            assert int(d_status.item()) == G.GCM_OK and np.array_equal(out.cpu().numpy(), pt)
+        finally:
+            G.gcm_destroy(ctx)
+
+
 def test_device_selection_and_current_device_untouched(G):
     """gcm_set_device only records the ordinal; contexts live on it (or on the caller's current device); no call
     changes the calling thread's current CUDA device."""
