@@ -143,7 +143,8 @@ GCM_API int gcm_measure_pipe_rates(double *rates, int n);
  * 8 x uint64 per CTA of the largest grid used (GCM_PHASE_SLOTS x grid x 8 bytes); while it is set, thread 0 of
  * every CTA stores %globaltimer (ns) at: [0] kernel entry, [1] tables in shared memory, [2] after
  * griddepcontrol.wait, [3] its rows done, [4] all warps' partials in, [5] ticket drawn, [6] finisher done (last CTA
- * only).  NULL switches it off (the default).  Not part of the data path.
+ * only), [7] position weights formed by warp 0 (between [1] and [2]).  NULL switches it off (the default).  Not part
+ * of the data path.
  */
 #define GCM_PHASE_SLOTS 8
 GCM_API int gcm_set_phase_stamps(gcm_ctx *ctx, void *d_stamps);
@@ -298,10 +299,12 @@ GCM_API int gcm_decrypt_verify_batch(gcm_msg *msgs, uint32_t n, void *cuda_strea
  * written into its own descriptor.  The caller fills the array once (keys included: it is the caller's to wipe) and
  * may launch it any number of times.
  *   key       16 or 32 bytes used          key_bits  128 or 256 (anything else: status = GCM_ERR_ARG, message skipped)
- *   tag       out (encrypt) / in (decrypt) status    out: GCM_OK / GCM_ERR_AUTH (output zero-filled) / GCM_ERR_ARG
+ *   tag       out (encrypt) / in (decrypt) status    out: GCM_OK / GCM_ERR_AUTH (output zero-filled) / GCM_ERR_ARG / GCM_ERR_LEN
  *   iv        12 bytes                     d_aad / d_in / d_out (device), aad_len, len as in gcm_msg
  * Every message is handled by one warp whatever its length: meant for messages up to a few hundred KiB (longer ones
- * are correct but slow; use gcm_encrypt_batch for FITS-sized messages).  Length limits and overlap rules are the
+ * are correct but slow; use gcm_encrypt_batch for FITS-sized messages).  The ordering kernel checks what it can see
+ * of each descriptor: len > 2^36 - 32 or aad_len >= 2^36 gives status GCM_ERR_LEN, a NULL d_in / d_out / d_aad with
+ * a non-zero length GCM_ERR_ARG, and such messages are skipped like one with a bad key_bits.  Overlap rules are the
  * caller's to keep (the descriptors cannot be checked from the host).  Calls on different streams are ordered behind
  * each other by the library.  Returns GCM_OK or a negative error for the launch itself.
  */

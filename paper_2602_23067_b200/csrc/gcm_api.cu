@@ -110,12 +110,6 @@ extern "C" const char *gcm_last_cuda_error_string(void)
     return cudaGetErrorString((cudaError_t)g_last_cuda_error.load());
 }
 
-static void secure_zero(void *p, size_t n)      // memset the compiler may not drop
-{
-    memset(p, 0, n);
-    __asm__ __volatile__("" : : "r"(p) : "memory");
-}
-
 static SetupParams setup_params(gcm_ctx *c, const uint8_t *key)
 {
     SetupParams sp;

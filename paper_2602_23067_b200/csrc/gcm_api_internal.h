@@ -2,7 +2,16 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 #include <atomic>
+
+// memset that the compiler may not drop as a dead store (parameter blocks hold round keys, staging holds raw keys;
+// runs at memory speed, not byte by byte)
+static inline void secure_zero(void *p, size_t n)
+{
+    memset(p, 0, n);
+    __asm__ __volatile__("" : : "r"(p) : "memory");
+}
 
 struct HostPipe;          // gcm_host.cu: staging buffers, streams and events of the host-buffer entry points
 

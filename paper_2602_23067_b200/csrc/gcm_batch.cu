@@ -24,10 +24,6 @@
 #include <cuda_runtime.h>
 #include <string.h>
 #include <stddef.h>
-#ifdef GCM_PIPE_DEBUG
-#include <chrono>
-#include <stdio.h>
-#endif
 #include <algorithm>
 #include <map>
 #include <mutex>
@@ -255,9 +251,21 @@ static cudaError_t launch_batch(int blocks, const BatchDesc *descs, uint8_t *res
 
 // Device-descriptor calls: ticket order (longest first, by 512-byte rows) for the two key sizes, made on the device.
 // One CTA: histogram over (key size, row count), exclusive scan, scatter.  order[0 .. n) holds the AES-128 messages,
-// order[n .. 2n) the AES-256 ones; counts[0 / 1] how many of each; descriptors with any other key_bits get
-// status GCM_ERR_ARG and are left out.  ctr[0..3] = ticket counters and counts, zeroed / written here.
+// order[n .. 2n) the AES-256 ones; counts[0 / 1] how many of each; descriptors with any other key_bits, a length
+// beyond the limits or a NULL buffer get status GCM_ERR_ARG / GCM_ERR_LEN and are left out.  ctr[0..3] = ticket counters and counts, zeroed / written here.
 #define ORDER_BUCKETS 514
+// What a device-resident descriptor can be refused for before any warp touches it: 0 = take it.  A message longer than
+// 2^36 - 32 bytes would wrap the 32-bit counter and reuse keystream (SP 800-38D limit, include/gcm.h); an AAD of 2^36
+// bytes or more overflows the 32-bit AAD block count of the row layout; a NULL buffer with a non-zero length would
+// fault the launch for every message of the batch.
+__device__ __forceinline__ int batch_desc_refusal(const BatchDesc &d)
+{
+    if (d.key_bits != 128 && d.key_bits != 256) return GCM_ERR_ARG;
+    if (d.len > ((1ull << 36) - 32) || d.aad_len >= (1ull << 36)) return GCM_ERR_LEN;
+    if ((d.len && (!d.in || !d.out)) || (d.aad_len && !d.aad)) return GCM_ERR_ARG;
+    return 0;
+}
+
 __global__ void __launch_bounds__(1024, 1)
 gcm_batch_order_kernel(BatchDesc *descs, uint32_t n, uint32_t *order, unsigned *ctr)
 {
@@ -271,12 +279,12 @@ gcm_batch_order_kernel(BatchDesc *descs, uint32_t n, uint32_t *order, unsigned *
         return (uint32_t)(ORDER_BUCKETS - 1 - (rows < ORDER_BUCKETS - 1 ? rows : ORDER_BUCKETS - 1));
     };
     for (uint32_t i = t; i < n; i += blockDim.x) {
-        const uint32_t kb = descs[i].key_bits;
-        if (kb == 128 || kb == 256) {
-            atomicAdd(&hist[kb == 256][bucket(descs[i].len)], 1u);
+        const int refusal = batch_desc_refusal(descs[i]);
+        if (refusal == 0) {
+            atomicAdd(&hist[descs[i].key_bits == 256][bucket(descs[i].len)], 1u);
             descs[i].status = GCM_STATUS_PENDING;          // reads "refused" until the message's warp has written it
         } else {
-            descs[i].status = GCM_ERR_ARG;
+            descs[i].status = refusal;
         }
     }
     __syncthreads();
@@ -287,9 +295,8 @@ gcm_batch_order_kernel(BatchDesc *descs, uint32_t n, uint32_t *order, unsigned *
     }
     __syncthreads();
     for (uint32_t i = t; i < n; i += blockDim.x) {
-        const uint32_t kb = descs[i].key_bits;
-        if (kb != 128 && kb != 256) continue;
-        const unsigned cls = kb == 256;
+        if (descs[i].status != GCM_STATUS_PENDING) continue;    // refused in the first pass (this thread wrote it)
+        const unsigned cls = descs[i].key_bits == 256;
         const unsigned pos = atomicAdd(&hist[cls][bucket(descs[i].len)], 1u);
         order[(size_t)cls * n + pos] = i;
     }
@@ -322,14 +329,6 @@ struct BatchState {
     size_t multi_cap = 0;
 };
 BatchState g;
-
-// memset that the compiler may not drop (the descriptor staging holds raw keys: 1 MB per 10,000 messages,
-// so this must run at memory speed, not byte by byte)
-void secure_zero(void *p, size_t n)
-{
-    memset(p, 0, n);
-    __asm__ __volatile__("" : : "r"(p) : "memory");
-}
 
 void free_staging_locked()
 {
@@ -553,16 +552,6 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     rc = ensure_staging_locked(n);
     if (rc != GCM_OK) return rc;
     if (g.dev_pending) { CUB(cudaStreamWaitEvent(s, g.dev_done, 0)); g.dev_pending = false; }
-#ifdef GCM_PIPE_DEBUG
-    auto T0 = std::chrono::steady_clock::now();
-    auto lap = [&](const char *what) {
-        auto t = std::chrono::steady_clock::now();
-        fprintf(stderr, "batch: %-10s %7.1f us\n", what, std::chrono::duration<double, std::micro>(t - T0).count());
-        T0 = t;
-    };
-#else
-    auto lap = [](const char *) {};
-#endif
 
     int first_err = GCM_OK;
     std::vector<uint32_t> small[2], large;                  // small[0]: AES-128, small[1]: AES-256
@@ -597,7 +586,6 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
             pos += count[k];
         }
     }
-    lap("marshal+sort");
     CUB(cudaMemcpyAsync(g.d_desc, g.h_desc, (size_t)n * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
     if (pos) CUB(cudaMemcpyAsync(g.d_order, g.h_order, (size_t)pos * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
     CUB(cudaMemsetAsync(g.d_next, 0, 2 * sizeof(unsigned), s));
@@ -620,9 +608,7 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
     // the descriptors hold raw keys: wipe the device copy on the stream, the host copy after the sync
     launch_wipe((uint8_t *)g.d_desc, (uint64_t)n * sizeof(BatchDesc), nullptr, s);
     CUB(cudaGetLastError());
-    lap("enqueue");
     CUB(cudaStreamSynchronize(s));
-    lap("gpu+sync");
     secure_zero(g.h_desc, (size_t)n * sizeof(BatchDesc));
     if (g.by_key.size() > BatchState::kMaxKeys) evict_keys_locked();     // nothing is in flight after the sync
     int failures = 0;
@@ -636,7 +622,6 @@ int run_batch(gcm_msg *msgs, uint32_t n, void *stream, bool decrypt)
             memcpy(m.tag, g.h_res[i].tag, 16);
         }
     }
-    lap("results");
     if (first_err != GCM_OK) return first_err;
     return decrypt ? failures : GCM_OK;
 }

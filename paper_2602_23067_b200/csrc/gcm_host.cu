@@ -11,12 +11,6 @@
 #include <cuda_runtime.h>
 #include <string.h>
 #include <new>
-#ifdef GCM_PIPE_DEBUG
-#include <chrono>
-#include <stdio.h>
-#include <stdlib.h>
-static cudaEvent_t dbg_ev[64][4];
-#endif
 
 #include "../../include/gcm.h"
 #include "gcm_common.cuh"
@@ -189,9 +183,13 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
     if (rc != GCM_OK) return rc;
     HostPipe *hp = c->pipe;
     cudaStream_t us = (cudaStream_t)user_stream;
-#ifdef GCM_PIPE_DEBUG
-    const auto t_begin = std::chrono::steady_clock::now();
-#endif
+    // An error return after the first enqueue must not leave copies in flight on the caller's h_in / h_out: every
+    // early return below drains the pipeline streams first (the success paths have synchronised already).
+    struct Drain {
+        HostPipe *hp;
+        bool armed;
+        ~Drain() { if (armed) for (int i = 0; i < PIPE_SLOTS; i++) cudaStreamSynchronize(hp->stream[i]); }
+    } drain{hp, true};
 
     // Short messages in pinned (or registered) host memory skip the staging copies altogether: under unified
     // addressing the kernel reads the plaintext and writes the ciphertext in place over PCIe, one launch, no DMA
@@ -216,9 +214,10 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
             p.tag_out = (uint4 *)c->h_pinned;
             p.status = (int *)(c->h_pinned + 16);
             cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s0);
-            memset(&p, 0, sizeof(p));
+            secure_zero(&p, sizeof(p));
             if (e != cudaSuccess) return gcm_cuda_fail(e);
             CU(cudaStreamSynchronize(s0));
+            drain.armed = false;
             if (mode == MODE_ENCRYPT) { memcpy(tag_io, c->h_pinned, 16); return GCM_OK; }
             if (*verdict0 != 0) { memset(h_out, 0, len); return GCM_ERR_AUTH; }
             return GCM_OK;
@@ -252,13 +251,7 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         cudaStream_t s = hp->stream[slot];
         const uint64_t clen = plan[k];
         const bool first = (k == 0), last = (k == n_chunks - 1);
-#ifdef GCM_PIPE_DEBUG
-        if (k < 64) { for (int q = 0; q < 4; q++) if (!dbg_ev[k][q]) cudaEventCreate(&dbg_ev[k][q]); cudaEventRecord(dbg_ev[k][0], s); }
-#endif
         if (clen) CU(cudaMemcpyAsync(hp->d_stage[slot], (const uint8_t *)h_in + off, clen, cudaMemcpyHostToDevice, s));
-#ifdef GCM_PIPE_DEBUG
-        if (k < 64) cudaEventRecord(dbg_ev[k][1], s);
-#endif
         // kernels run in message order: chunk k needs chunk k-1's GHASH state (and the powers)
         if (!first) CU(cudaStreamWaitEvent(s, hp->kernel_done[(k - 1) % PIPE_SLOTS], 0));
         else if (n_chunks > 1) CU(cudaStreamWaitEvent(s, hp->kernel_done[PIPE_SLOTS - 1], 0));
@@ -279,33 +272,14 @@ int gcm_host_run(gcm_ctx *c, int mode, const uint8_t *iv, const void *h_aad, uin
         p.tag_out = (uint4 *)c->h_pinned;
         p.status = (int *)(c->h_pinned + 16);
         cudaError_t e = gcm_launch_fused(c, mode, blocks, p, s);
-        memset(&p, 0, sizeof(p));
+        secure_zero(&p, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
         CU(cudaEventRecord(hp->kernel_done[slot], s));
-#ifdef GCM_PIPE_DEBUG
-        if (k < 64) cudaEventRecord(dbg_ev[k][2], s);
-#endif
         if (d_sum32 && mode == MODE_ENCRYPT) CU(launch_fits_sum32(hp->d_stage[slot], clen, d_sum32, c->sm_count, s));
         if (clen && mode != MODE_GHASH) CU(cudaMemcpyAsync((uint8_t *)h_out + off, hp->d_stage[slot], clen, cudaMemcpyDeviceToHost, s));
-#ifdef GCM_PIPE_DEBUG
-        if (k < 64) cudaEventRecord(dbg_ev[k][3], s);
-#endif
     }
-#ifdef GCM_PIPE_DEBUG
-    const double t_enq = std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count();
-#endif
     for (int i = 0; i < PIPE_SLOTS; i++) CU(cudaStreamSynchronize(hp->stream[i]));
-#ifdef GCM_PIPE_DEBUG
-    fprintf(stderr, "pipe: %u chunks, enqueue %.0f us, total %.0f us\n", n_chunks, t_enq,
-            std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t_begin).count());
-    if (getenv("GCM_PIPE_TIMELINE"))
-        for (uint32_t k = 0; k < n_chunks && k < 64; k++) {
-            float a, b, c2, d2;
-            cudaEventElapsedTime(&a, dbg_ev[0][0], dbg_ev[k][0]); cudaEventElapsedTime(&b, dbg_ev[0][0], dbg_ev[k][1]);
-            cudaEventElapsedTime(&c2, dbg_ev[0][0], dbg_ev[k][2]); cudaEventElapsedTime(&d2, dbg_ev[0][0], dbg_ev[k][3]);
-            fprintf(stderr, "  chunk %2u %6.2f MiB: h2d start %7.1f end %7.1f | kernel end %7.1f | d2h end %7.1f us\n", k, plan[k] / 1048576.0, a * 1e3, b * 1e3, c2 * 1e3, d2 * 1e3);
-        }
-#endif
+    drain.armed = false;
     if (mode != MODE_DECRYPT) {
         memcpy(tag_io, c->h_pinned, 16);
         return GCM_OK;
@@ -379,7 +353,7 @@ extern "C" int gcm_decrypt_verify_host_strict(gcm_ctx *c, const uint8_t iv[12], 
         c->ticket_next -= (unsigned)blocks;                      // the latency kernel draws no tickets
         p.tag_out = hp->d_state;                                 // E_K(J0)
         cudaError_t e = launch_small(c->nr, MODE_ENCRYPT, p, s);
-        memset(&p, 0, sizeof(p));
+        secure_zero(&p, sizeof(p));
         if (e != cudaSuccess) return gcm_cuda_fail(e);
     }
     CU(cudaMemcpyAsync(hp->d_state + 1, s_host, 16, cudaMemcpyHostToDevice, s));

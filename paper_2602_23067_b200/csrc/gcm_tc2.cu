@@ -24,6 +24,7 @@
 #include "gf128.cuh"
 #include "gcm_fused.cuh"
 #include "gcm_tc.cuh"
+#include "gcm_api_internal.h"
 
 #include "gcm_device.cuh"
 
@@ -396,7 +397,6 @@ cudaError_t launch_tc2(int nr, int mode, int blocks, const uint32_t *rk, const u
     cudaError_t e;
     if (nr == 10) e = mode == MODE_ENCRYPT ? tc2_launch_one<10, MODE_ENCRYPT>(blocks, p, s) : tc2_launch_one<10, MODE_DECRYPT>(blocks, p, s);
     else e = mode == MODE_ENCRYPT ? tc2_launch_one<14, MODE_ENCRYPT>(blocks, p, s) : tc2_launch_one<14, MODE_DECRYPT>(blocks, p, s);
-    volatile uint32_t *z = p.rk;
-    for (int i = 0; i < 60; i++) z[i] = 0;
+    secure_zero(&p, sizeof(p));
     return e;
 }

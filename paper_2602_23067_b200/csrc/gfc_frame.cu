@@ -505,8 +505,12 @@ extern "C" int gfc_encrypt_frame(gfc_context *c, const uint8_t *fits, uint64_t f
     const std::string aad = data_aad(nonce_d, o);
     CUF(cudaMemsetAsync(d_sum, 0, 8, c->streamD));
     CUF(cudaEventRecord(c->evD0, c->streamD));
-    rc = gcm_host_run(c->g[1], MODE_ENCRYPT, nonce_d, aad.data(), aad.size(), fits + hlen, n, c->h_out + L0 + L1, tag_d,
-                      c->streamD, d_sum);
+    {
+        CtxLock lock(c->g[1]);                  // gcm_host_run wants the key context's lock held (one call at a time)
+        if (!lock.ok) return fail(res, GCM_ERR_BUSY, "data key context is in use");
+        rc = gcm_host_run(c->g[1], MODE_ENCRYPT, nonce_d, aad.data(), aad.size(), fits + hlen, n, c->h_out + L0 + L1, tag_d,
+                          c->streamD, d_sum);
+    }
     if (rc != GCM_OK) return fail(res, rc, "data message failed");
     CUF(cudaMemcpyAsync(c->h_small + 64, d_sum, 8, cudaMemcpyDeviceToHost, c->streamD));
     CUF(cudaEventRecord(c->evD1, c->streamD));
@@ -594,7 +598,11 @@ extern "C" int gfc_decrypt_frame(gfc_context *c, const uint8_t *ctr, uint64_t le
         if (rc != GCM_OK) return fail(res, rc, "data key setup failed");
         const std::string aad = data_aad(nonce_d, o);
         CUF(cudaEventRecord(c->evD0, c->streamD));
-        rc = gcm_host_run(c->g[1], MODE_DECRYPT, nonce_d, aad.data(), aad.size(), ctr + d_off, n, pay, tag_d, c->streamD, nullptr);
+        {
+            CtxLock lock(c->g[1]);
+            if (!lock.ok) return fail(res, GCM_ERR_BUSY, "data key context is in use");
+            rc = gcm_host_run(c->g[1], MODE_DECRYPT, nonce_d, aad.data(), aad.size(), ctr + d_off, n, pay, tag_d, c->streamD, nullptr);
+        }
         if (rc < 0) return fail(res, rc, "data message failed");
         CUF(cudaEventRecord(c->evD1, c->streamD));
         CUF(cudaStreamSynchronize(c->streamD));

@@ -247,6 +247,14 @@ def test_batch_device_descriptors(G, oracle):
     assert host.dtype.itemsize == G.GCM_DMSG_BYTES == 112
     bad = len(msgs) // 2
     host["key_bits"][bad] = 192                                   # not a key size of reading S1
+    # descriptors the ordering kernel must refuse without touching their buffers: a length that would wrap the 32-bit
+    # counter, an AAD length beyond the row layout, NULL buffers with non-zero lengths
+    refused = {bad: G.GCM_ERR_ARG}
+    for i, (field, value, code) in zip([3, 11, 12, 13, 15], [("len", (1 << 36) - 31, G.GCM_ERR_LEN), ("aad_len", 1 << 36, G.GCM_ERR_LEN),
+                                                          ("d_in", 0, G.GCM_ERR_ARG), ("d_out", 0, G.GCM_ERR_ARG), ("d_aad", 0, G.GCM_ERR_ARG)]):
+        assert len(specs[i][3]) > 0 and (field != "d_aad" or len(specs[i][2]) > 0)
+        host[field][i] = value
+        refused[i] = code
     d_msgs = torch.from_numpy(host.view(np.uint8).copy()).cuda()
     for _ in range(2):                                            # the same descriptor array twice
         G.gcm_encrypt_batch_device(d_msgs)
@@ -258,8 +266,8 @@ def test_batch_device_descriptors(G, oracle):
     for i, ((key, iv, aad, pt, _), o) in enumerate(zip(specs, offs)):
         ref_ct, ref_tag = oracle.gcm_encrypt(key, iv, aad, pt)
         refs.append((ref_ct, ref_tag))
-        if i == bad:
-            assert int(res["status"][i]) == G.GCM_ERR_ARG
+        if i in refused:
+            assert int(res["status"][i]) == refused[i], i
             assert not out[o: o + len(pt)].any(), "a refused descriptor was processed"
             continue
         assert int(res["status"][i]) == G.GCM_OK, i
