@@ -479,6 +479,15 @@ def run_ours(args):
             e2e["frac"] = e2e["value"] / world / link["per_direction_duplex"]
             e2e["pcie"] = link
 
+    # the SM clock the dominant kernel really ran at in the last timed step, from the kernel's own clock64 / %globaltimer
+    kernel_clock = None
+    if rank == 0 and n >= G.TC2_AUTO_BYTES[256]:
+        try:
+            mhz, k_ms = G.gcm_debug_tc2_clock(ctx)
+            kernel_clock = {"sm_mhz": mhz, "kernel_ms": k_ms}
+        except G.GcmError:
+            kernel_clock = None
+
     # the shared-memory table kernel on the same message, beside it (not the reported value)
     table_engine = None
     if rank == 0 and n >= G.TC2_AUTO_BYTES[256]:
@@ -545,6 +554,16 @@ def run_ours(args):
         if clocks.get("sm_mhz"):
             roofline["frac_self_derived_at_sampled_clock"] = roofline["frac_at_sampled_clock"]
             roofline["frac_at_sampled_clock"] = roofline["frac"] * sm_mhz / clocks["sm_mhz"]
+        if kernel_clock:
+            # nvidia-smi (clocks.sm_mhz) keeps showing the maximum while a tcgen05 kernel runs below it: the kernel's own
+            # cycle and nanosecond counters (gcm_debug_tc2_clock, CTA 0 of the last timed step) give the clock that applies
+            roofline["sm_mhz_kernel"] = kernel_clock["sm_mhz"]
+            roofline["kernel_ms_by_globaltimer"] = kernel_clock["kernel_ms"]
+            roofline["frac_at_kernel_clock"] = roofline["frac"] * sm_mhz / kernel_clock["sm_mhz"]
+            roofline["frac_self_derived_at_kernel_clock"] = roofline["frac_self_derived"] * sm_mhz / kernel_clock["sm_mhz"]
+            roofline["frac_at_sampled_clock"] = roofline["frac_at_kernel_clock"]
+            roofline["sampled_clock_note"] = ("frac_at_sampled_clock uses sm_mhz_kernel (measured inside the kernel); nvidia-smi sampled %s MHz"
+                                              % clocks.get("sm_mhz"))
         roofline["pipe"] = ("shared-memory data pipe (LSU): %.1f wavefront-lanes per 16-byte block measured for the launch (%s): AES table reads, "
                             "the hand-over of the ciphertext to the GHASH warps, and the tensor core's reads of the bit matrices; 32 per SM-cycle. "
                             "GHASH itself runs on tcgen05.mma kind::mxf4" % (pb["lanes_per_block"], pb["mix"]))

@@ -173,6 +173,18 @@ typedef struct {
 GCM_API int gcm_debug_row_layout(uint64_t len, uint64_t aad_len, uint32_t ctr_base, int last, int aligned, gcm_row_layout *out);
 GCM_API int gcm_debug_plan_chunks(uint64_t len, uint64_t *plan, uint32_t cap);
 
+/*
+ * Diagnostics: the SM clock the tensor-core kernel of the long-message path (gcm_tc2_kernel) ran at in
+ * this context's most recent call, measured by the kernel itself: CTA 0 stores clock64() and %globaltimer at its entry
+ * and exit into the context's scratch (four words, always, not a data-path branch).  nvidia-smi keeps reporting the
+ * maximum clock while a tcgen05 kernel runs several per cent below it, so the roofline of bench.py uses this value.
+ *   sm_mhz     host, out: SM cycles per microsecond over CTA 0's lifetime
+ *   kernel_ms  host, out: that lifetime in milliseconds
+ * Synchronises the device.  Returns GCM_OK, GCM_ERR_ARG (NULL argument, or no such kernel has run on the context),
+ * GCM_ERR_BUSY or GCM_ERR_CUDA.
+ */
+GCM_API int gcm_debug_tc2_clock(gcm_ctx *ctx, double *sm_mhz, double *kernel_ms);
+
 /* Copies the hash subkey H = E_K(0^128) (16 bytes) to host memory; for tests of step a2. */
 GCM_API int gcm_get_hash_subkey(const gcm_ctx *ctx, uint8_t h[16]);
 

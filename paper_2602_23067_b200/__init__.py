@@ -12,7 +12,7 @@ _BINDING_NAMES = (
     "gcm_get_geometry", "gcm_set_ghash_engine", "gcm_get_ghash_engine", "GCM_GHASH_TABLE", "GCM_GHASH_TENSOR", "GCM_GHASH_AUTO", "TC2_AUTO_BYTES", "GHASH_TC_AUTO_BYTES", "gcm_get_hash_subkey", "gcm_encrypt", "gcm_decrypt_verify",
     "gcm_encrypt_async", "gcm_decrypt_verify_async", "gcm_ghash_async", "gcm_encrypt_host",
     "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps", "gcm_encrypt_batch", "gcm_decrypt_verify_batch",
-    "MsgBatch", "gcm_pack_msgs", "gcm_batch_release", "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_pack_dmsgs", "gcm_debug_row_layout", "gcm_debug_plan_chunks", "gcm_dmsg_dtype", "GCM_DMSG_BYTES", "gcm_measure_pipe_rates", "RATE_NAMES", "library_path", "EXPORTED_SYMBOLS",
+    "MsgBatch", "gcm_pack_msgs", "gcm_batch_release", "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_pack_dmsgs", "gcm_debug_row_layout", "gcm_debug_plan_chunks", "gcm_debug_tc2_clock", "gcm_dmsg_dtype", "GCM_DMSG_BYTES", "gcm_measure_pipe_rates", "RATE_NAMES", "library_path", "EXPORTED_SYMBOLS",
 )
 __all__ = list(_BINDING_NAMES)
 

@@ -165,7 +165,7 @@ int gcm_init_on_device(gcm_ctx **out, const uint8_t *key, int key_bits, int devi
     size_t o_hpow = take((GCM_STRIDE + 1) * 16), o_hx = take(HX_ENTRIES * 16);
     size_t o_ktab = take(KTAB_BYTES), o_part = take(GCM_MAX_GRID * 16);
     size_t o_cnt = take(4), o_tag = take(16), o_status = take(4), o_bmat = take(TC_BMAT_TOTAL);
-    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES), o_gt = take(64);
+    size_t o_bmat2 = take(GT_BMAT_TOTAL), o_ktab2 = take(KTAB_BYTES), o_gt = take(128);   // d_gt[0..2]: chain state; bytes 64..95: clock probe of gcm_tc2_kernel
     c->slab_bytes = off;
     cudaError_t e = cudaSuccess;
     {
@@ -464,7 +464,8 @@ static int crypt_tc2_locked(gcm_ctx *c, int mode, const uint8_t iv[12], const vo
     blocks = (int)(nslices < (uint64_t)c->grid ? nslices : (uint64_t)c->grid);
     c->ticket_next += (unsigned)blocks;
     e = launch_tc2(c->nr, mode, blocks, c->h_rk, c->h_te0, iv, T2_HEAD_BLOCKS + 2, in + head, out + head, nslices, c->d_bmat2, c->d_hx,
-                   c->d_partials, c->d_counter, c->ticket_next - 1, c->d_gt + 0, c->d_gt + 1, (tail + 15) / 16 + 1, c->d_gt + 2, s);
+                   c->d_partials, c->d_counter, c->ticket_next - 1, c->d_gt + 0, c->d_gt + 1, (tail + 15) / 16 + 1, c->d_gt + 2,
+                   reinterpret_cast<unsigned long long *>(c->d_gt + 4), s);
     if (e != cudaSuccess) { c->ticket_next -= (unsigned)blocks; return gcm_cuda_fail(e); }
     rc = gcm_build_params(c, mode, iv, nullptr, 0, in + head + bulk, tail, out + head + bulk, (uint32_t)(T2_HEAD_BLOCKS + 128 * nslices), true,
                           len, aad_len, &p, &blocks);
@@ -613,5 +614,20 @@ extern "C" int gcm_decrypt_verify(gcm_ctx *c, const uint8_t iv[12], const void *
         CU(cudaStreamSynchronize((cudaStream_t)stream));
         return GCM_ERR_AUTH;
     }
+    return GCM_OK;
+}
+
+// Diagnostics: the SM clock gcm_tc2_kernel ran at in the context's most recent chain (CTA 0's clock64 and %globaltimer
+// at entry and exit, left in the context's scratch by the kernel itself).  Synchronises the device.
+extern "C" int gcm_debug_tc2_clock(gcm_ctx *c, double *sm_mhz, double *kernel_ms)
+{
+    if (!c || !sm_mhz || !kernel_ms) return GCM_ERR_ARG;
+    LOCK_CTX(c);
+    unsigned long long v[4] = {0, 0, 0, 0};
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(v, c->d_gt + 4, sizeof(v), cudaMemcpyDeviceToHost));
+    if (v[3] <= v[1] || v[2] <= v[0]) return GCM_ERR_ARG;          // no gcm_tc2 launch on this context yet
+    *sm_mhz = (double)(v[2] - v[0]) / (double)(v[3] - v[1]) * 1e3;  // cycles per ns -> MHz
+    *kernel_ms = (double)(v[3] - v[1]) * 1e-6;
     return GCM_OK;
 }

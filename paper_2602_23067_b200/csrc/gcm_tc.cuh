@@ -24,4 +24,4 @@ cudaError_t launch_ghash_tc(int blocks, const uint8_t *aad, uint64_t aad_len, co
 cudaError_t launch_tc2(int nr, int mode, int blocks, const uint32_t *rk, const uint32_t *te0, const uint8_t *iv, uint32_t ctr0,
                        const uint8_t *in, uint8_t *out, uint64_t nslices, const uint4 *bmat2, const uint4 *hx, uint4 *partials,
                        unsigned *counter, unsigned ticket_last, const uint4 *chain_in, uint4 *chain_out, uint64_t exp_next,
-                       uint4 *pow_out, cudaStream_t s);
+                       uint4 *pow_out, unsigned long long *clk, cudaStream_t s);

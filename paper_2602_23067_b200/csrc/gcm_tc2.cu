@@ -64,6 +64,7 @@ struct Tc2Params {
     uint4    *chain_out;        // state behind it
     uint64_t  exp_next;         // H^exp_next goes to pow_out: chain_pow of the launch that follows
     uint4    *pow_out;
+    unsigned long long *clk;    // diagnostics, or NULL: CTA 0 leaves {clock64, %globaltimer} of its entry and exit here (4 words)
 };
 
 __device__ __forceinline__ void t2_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -176,6 +177,9 @@ gcm_tc2_kernel(const __grid_constant__ Tc2Params p)
     const uint32_t T = (uint32_t)(s1 - s0);
     if (warp == T2_AES + 4) {
         if (lane == 0) {
+            // SM clock this kernel really runs at (the tensor pipe lowers it below what nvidia-smi reports): cycles and
+            // nanoseconds of CTA 0's life, stored at once so that no register is held across the AES warps' loop
+            if (blockIdx.x == 0 && p.clk != nullptr) { p.clk[0] = (unsigned long long)clock64(); p.clk[1] = global_timer_ns(); }
             uint64_t *b = reinterpret_cast<uint64_t *>(sm + T2_BAR_OFF);
             mbar_init(b + 0, 1);
             for (int i = 0; i < T2_STAGES; i++) { mbar_init(b + 1 + i, 1); mbar_init(b + 1 + T2_STAGES + i, 4); }
@@ -353,6 +357,7 @@ gcm_tc2_kernel(const __grid_constant__ Tc2Params p)
         const uint64_t behind = (p.nslices - s1) * 128;
         if (behind && T) acc = gf_mul_mem(acc, red[4]);
         pdl_wait();
+        if (blockIdx.x == 0 && p.clk != nullptr) { p.clk[2] = (unsigned long long)clock64(); p.clk[3] = global_timer_ns(); }
         p.partials[blockIdx.x] = acc;
         asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(p.counter) : "memory");
     }
@@ -384,7 +389,7 @@ static cudaError_t tc2_launch_one(int blocks, const Tc2Params &p, cudaStream_t s
 cudaError_t launch_tc2(int nr, int mode, int blocks, const uint32_t *rk, const uint32_t *te0, const uint8_t *iv, uint32_t ctr0,
                        const uint8_t *in, uint8_t *out, uint64_t nslices, const uint4 *bmat2, const uint4 *hx, uint4 *partials,
                        unsigned *counter, unsigned ticket_last, const uint4 *chain_in, uint4 *chain_out, uint64_t exp_next,
-                       uint4 *pow_out, cudaStream_t s)
+                       uint4 *pow_out, unsigned long long *clk, cudaStream_t s)
 {
     Tc2Params p;
     memset(&p, 0, sizeof(p));
@@ -393,7 +398,7 @@ cudaError_t launch_tc2(int nr, int mode, int blocks, const uint32_t *rk, const u
     memcpy(p.iv, iv, 12);
     p.ctr0 = ctr0; p.in = in; p.out = out; p.nslices = nslices; p.bmat2 = bmat2; p.hx = hx;
     p.partials = partials; p.counter = counter; p.ticket_last = ticket_last;
-    p.chain_in = chain_in; p.chain_out = chain_out; p.exp_next = exp_next; p.pow_out = pow_out;
+    p.chain_in = chain_in; p.chain_out = chain_out; p.exp_next = exp_next; p.pow_out = pow_out; p.clk = clk;
     cudaError_t e;
     if (nr == 10) e = mode == MODE_ENCRYPT ? tc2_launch_one<10, MODE_ENCRYPT>(blocks, p, s) : tc2_launch_one<10, MODE_DECRYPT>(blocks, p, s);
     else e = mode == MODE_ENCRYPT ? tc2_launch_one<14, MODE_ENCRYPT>(blocks, p, s) : tc2_launch_one<14, MODE_DECRYPT>(blocks, p, s);

@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = [
     "gcm_encrypt", "gcm_decrypt_verify", "gcm_encrypt_async", "gcm_decrypt_verify_async",
     "gcm_encrypt_host", "gcm_decrypt_verify_host", "gcm_decrypt_verify_host_strict", "gcm_set_phase_stamps",
     "gcm_ghash_async", "gcm_encrypt_batch", "gcm_decrypt_verify_batch", "gcm_batch_release",
-    "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_debug_row_layout", "gcm_debug_plan_chunks",
+    "gcm_encrypt_batch_device", "gcm_decrypt_verify_batch_device", "gcm_debug_row_layout", "gcm_debug_plan_chunks", "gcm_debug_tc2_clock",
     "gcm_measure_pipe_rates",
 ]
 RATE_NAMES = ["lds32", "lds128", "lop3", "prmt", "imad", "imad_wide", "lop3_imad", "mma_mxf4_blocks"]
@@ -108,6 +108,7 @@ def _load() -> ctypes.CDLL:
     L.gcm_decrypt_verify_batch_device.argtypes = [vp, ctypes.c_uint32, vp]
     L.gcm_debug_row_layout.argtypes = [u64, u64, ctypes.c_uint32, ci, ci, ctypes.POINTER(GcmRowLayout)]
     L.gcm_debug_plan_chunks.argtypes = [u64, ctypes.POINTER(u64), ctypes.c_uint32]
+    L.gcm_debug_tc2_clock.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.gcm_batch_release.argtypes = []
     L.gcm_batch_release.restype = None
     L.gcm_measure_pipe_rates.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_int]
@@ -479,6 +480,13 @@ def gcm_debug_row_layout(length: int, aad_len: int, ctr_base: int = 0, last: boo
     _check(_L.gcm_debug_row_layout(length, aad_len, ctr_base, 1 if last else 0, 1 if aligned else 0, ctypes.byref(out)),
            "gcm_debug_row_layout")
     return {k: getattr(out, k) for k, _ in GcmRowLayout._fields_ if k != "reserved"}
+
+
+def gcm_debug_tc2_clock(ctx: int) -> Tuple[float, float]:
+    """(SM MHz, kernel ms) of gcm_tc2_kernel in the context's most recent long-message call, measured by the kernel."""
+    mhz, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(_L.gcm_debug_tc2_clock(ctx, ctypes.byref(mhz), ctypes.byref(ms)), "gcm_debug_tc2_clock")
+    return float(mhz.value), float(ms.value)
 
 
 def gcm_debug_plan_chunks(length: int) -> List[int]:

@@ -403,3 +403,28 @@ def test_tensor_kernels_of_several_contexts_on_several_streams(G, oracle):
     finally:
         for _, ctx, _ in jobs:
             G.gcm_destroy(ctx)
+
+
+def test_tc2_kernel_reports_its_own_clock(G):
+    """gcm_debug_tc2_clock: refused before the context has run a gcm_tc2 chain; afterwards the SM clock measured by the
+    kernel itself (clock64 against %globaltimer over CTA 0's life) is a plausible B200 clock and its duration is
+    below the host-timed duration of the whole call."""
+    import time
+    ctx = G.gcm_init(bytes(range(32)))
+    try:
+        with pytest.raises(G.GcmError) as e:
+            G.gcm_debug_tc2_clock(ctx)
+        assert e.value.code == G.GCM_ERR_ARG
+        G.gcm_set_ghash_engine(ctx, G.GCM_GHASH_TENSOR)
+        n = 64 << 20
+        pt = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        ct = torch.empty_like(pt)
+        G.gcm_encrypt(ctx, bytes(12), None, pt, ct)                     # warm
+        t0 = time.perf_counter()
+        G.gcm_encrypt(ctx, bytes(12), None, pt, ct)
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        mhz, ms = G.gcm_debug_tc2_clock(ctx)
+        assert 1000.0 < mhz < 2300.0, mhz
+        assert 0.0 < ms < wall_ms, (ms, wall_ms)
+    finally:
+        G.gcm_destroy(ctx)
