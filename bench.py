@@ -140,6 +140,18 @@ def load_mix(key: str) -> dict:
                          "is derived from the shipped binary's executed mix and is not guessed" % (MIX_FILE, key, e))
 
 
+def mix_matches_library(key: str):
+    """True / False: the mix entry was captured from the very library file that is loaded now (size and SHA-256 stored
+    by profile_tools mix); None when the entry predates that record."""
+    import hashlib
+    fp = load_mix(key).get("library")
+    if not fp:
+        return None
+    import paper_2602_23067_b200 as G
+    data = open(G.library_path(), "rb").read()
+    return fp.get("bytes") == len(data) and fp.get("sha256") == hashlib.sha256(data).hexdigest()
+
+
 def pipe_bound_gbs(key: str, nr: int, sm_count: int, sm_mhz: float, rates: dict = None, ghash_only: bool = False) -> dict:
     """Shared-memory-pipe (LSU data pipe) bound.  An SM retires one 128-byte shared-memory wavefront per cycle: a
     conflict-free LDS.32 of a warp is one wavefront, an LDS.64 two, an LDS.128 four; a warp-row is 32 blocks, one per
@@ -536,6 +548,7 @@ def run_ours(args):
         "kernel": "gcm_tc2_kernel<14, ENCRYPT> (+ two short gcm_fused_kernel links)" if uses_tc2 else "gcm_fused_kernel<14, ENCRYPT, 512>",
         "kernel_ms_mean": kernel_ms,
         "kernel_ms_median": statistics.median(per),
+        "mix_captured_from_loaded_library": mix_matches_library(mix_key),
     })
     if clocks.get("sm_mhz"):
         roofline["frac_at_sampled_clock"] = achieved / pipe_bound_gbs(mix_key, 14, sm_count, clocks["sm_mhz"])["gbs"]

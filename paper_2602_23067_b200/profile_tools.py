@@ -83,6 +83,15 @@ def summary(report: str, out: str, command: str) -> None:
             f.write("\n")
 
 
+def _library_fingerprint() -> dict:
+    """Size and SHA-256 of the built libb200gcm.so next to this file: the binary the report was captured from (the
+    capture and this step run on the same build).  bench.py compares it with the library it has loaded."""
+    import hashlib
+    lib = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libb200gcm.so")
+    data = open(lib, "rb").read()
+    return {"bytes": len(data), "sha256": hashlib.sha256(data).hexdigest()}
+
+
 def mix(report: str, out: str, key: str, command: str) -> None:
     """Per-warp-row executed instruction mix of the FIRST kernel in the report."""
     text = _ncu_page(report, "source")
@@ -144,6 +153,14 @@ def mix(report: str, out: str, key: str, command: str) -> None:
             wf_total = float(raw[2][raw[0].index("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum")])
         except ValueError:
             wf_total = 0.0
+    # the launch's executed warp instructions from the hardware counter (the source page's per-line counts of the helper
+    # warps' polling loops are sampled differently and do not add up to it: use this one for issue-rate arithmetic)
+    inst_executed = 0.0
+    if len(raw) > 2 and "smsp__inst_executed.sum" in raw[0]:
+        try:
+            inst_executed = float(raw[2][raw[0].index("smsp__inst_executed.sum")])
+        except ValueError:
+            inst_executed = 0.0
     # one STG.E.EF.128 (streaming store of a full row) per fast warp-row; the slow rows are a rounding error at the
     # sizes this is captured on.  GHASH-only launches store nothing: there a row is one streaming LDG.128.
     stream_st = sum(v for k, v in by_op.items() if k.startswith("STG") and ".EF" in k and ".128" in k)
@@ -153,12 +170,13 @@ def mix(report: str, out: str, key: str, command: str) -> None:
         raise SystemExit("no streaming 128-bit store / load found: not a row-loop kernel?")
     per_row = lambda x: x / warp_rows
     entry = {
-        "kernel": kernel, "command": command, "warp_rows": warp_rows,
+        "kernel": kernel, "command": command, "warp_rows": warp_rows, "library": _library_fingerprint(),
         "per_warp_row": {
             "lds32": per_row(lds32), "lds64": per_row(lds64), "lds128": per_row(lds128),
             "ldg128": per_row(ldg128), "stg128": per_row(stg128), "sts128": per_row(sts128),
             "shared_wavefronts_total": per_row(wf_total),
             "warp_instructions": per_row(total), "warp_instructions_issued": per_row(issued),
+            "warp_instructions_executed_counter": per_row(inst_executed),
             "by_pipe_warp_instructions": {k: per_row(v) for k, v in sorted(by_pipe.items())},
             "shared_wavefronts": per_row(wf_shared), "shared_wavefronts_ideal": per_row(wf_shared_ideal),
             "top_opcodes": {k: round(per_row(v), 2) for k, v in by_op.most_common(24)},
